@@ -1,0 +1,179 @@
+/*
+ * pwa.h - C ABI of the B200-native partial-wave-analysis likelihood library (libpwa_b200.so).
+ *
+ * What the library computes (all arithmetic fp64, on one CUDA device, in hand-written sm_100a kernels):
+ *
+ *   intensity   I_i = sum_h | sum_r z_r(i) F_rh(i) |^2                      PAPER.md:57-60 (Eq. 1, 1/2 dropped:
+ *                                                                            DESIGN.md reading S1)
+ *   z_r(i) = a_r e^{i phi_r} / (M_r^2 - m_{ch(r)}(i)^2 - i M_r Gamma_r)      BASELINE.json configs[0] (S4)
+ *   NLL(theta) = - sum_data w_i ln I_i + W ln( sum_mc I_j / N_mc ),  W = sum_data w_i
+ *                                                                            PAPER.md:67 (Eq. 3), S2, S3
+ *   grad NLL, and (Hessian of NLL) . v for a given direction v               PAPER.md:90 (Eq. 6), :95 (Eq. 7, S9)
+ *   a truncated line-search Newton-CG minimisation of NLL                    PAPER.md:27, :119; DESIGN.md (c-F)
+ *
+ * Parameters: theta[4r..4r+3] = (a_r, phi_r, M_r, Gamma_r), r = 0..n_res-1 (S6); P = 4*n_res doubles.
+ * F_rh(i) ("amp") is the parameter-free projection of PAPER.md:70, an input computed once by the caller.
+ *
+ * Conventions
+ *   - Every call returns a pwa_status; nothing throws across this boundary; no global state except a
+ *     process-wide count of live handles.  One handle = one device + one stream; a handle is not
+ *     thread-safe, different handles are independent.
+ *   - There is no CPU path.  If no CUDA device is usable, pwa_create fails with PWA_ERR_CUDA.
+ *   - Evaluation calls (pwa_nll ... pwa_raw_sums, pwa_combine) only ENQUEUE work on the handle's stream
+ *     and return; they never synchronise.  Their theta / v / output pointers are DEVICE pointers that
+ *     must stay valid until the stream has run the work.  Outputs may not alias inputs.
+ *   - pwa_fit_newton_cg, pwa_status_flags and the *_host convenience calls synchronise the stream.
+ *   - Results are bit-identical between repeated calls with identical inputs on the same device
+ *     (fixed grid, fixed event -> thread map, fixed-order reductions, no floating-point atomics).
+ */
+#ifndef PWA_B200_H
+#define PWA_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PWA_MAX_RES 512   /* n_res  <= 512 */
+#define PWA_MAX_HEL 8     /* n_hel  <= 8   */
+#define PWA_MAX_CHAN 16   /* n_chan <= 16  */
+
+typedef struct pwa_handle pwa_handle; /* opaque, owned by the library */
+
+typedef enum {
+  PWA_OK = 0,
+  PWA_ERR_INVALID_ARG = 1,   /* null pointer, size out of range, misaligned buffer, bad res_chan ... */
+  PWA_ERR_CUDA = 2,          /* a CUDA runtime call failed (see pwa_last_error) or no device */
+  PWA_ERR_OOM = 3,           /* device (or pinned host) allocation failed */
+  PWA_ERR_NONFINITE = 4,     /* fit: NLL or gradient not finite at the start point */
+  PWA_ERR_NOT_CONVERGED = 5  /* fit: stopped without meeting the convergence classification (S19) */
+} pwa_status;
+
+typedef enum { PWA_MEM_HOST = 0, PWA_MEM_DEVICE = 1 } pwa_memkind;
+
+/* One event sample (data or phase-space MC).  Layouts (event index fastest):
+ *   mass  [n_chan][stride]            fp64, invariant mass m_c(i) in GeV of channel c
+ *   amp   [n_res][n_hel][stride][2]   fp64, (Re, Im) of F_rh(i), amplitude-major, interleaved complex
+ *   weight[n_events] or NULL          fp64, NULL = unit weights
+ * `stride` is the distance in EVENTS between consecutive planes (>= n_events; 0 means n_events). */
+typedef struct {
+  int64_t n_events;
+  int64_t stride;
+  const double* mass;
+  const double* amp;
+  const double* weight;
+} pwa_sample;
+
+typedef struct {
+  int32_t n_res, n_hel, n_chan;
+  const int32_t* res_chan; /* [n_res] HOST pointer, channel of each resonance, values in [0, n_chan) */
+  pwa_sample data, mc;     /* mc.weight must be NULL (unweighted phase space, S10) */
+  pwa_memkind mem;         /* where data/mc mass, amp, weight live */
+  int32_t borrow;          /* PWA_MEM_DEVICE only. 1: adopt the device pointers (zero copy; the caller
+                              keeps them alive and unchanged for the life of the handle; amp must be
+                              16-byte aligned, mass/weight 8-byte aligned).  0: the library copies and
+                              the caller may free its buffers when pwa_create returns. */
+  int32_t device;          /* CUDA device ordinal */
+  void* stream;            /* cudaStream_t, or NULL for the legacy default stream */
+} pwa_model_desc;
+
+/* Creates a handle: validates the descriptor (PWA_ERR_INVALID_ARG on: null desc/out/res_chan/mass/amp,
+ * n_res not in [1,PWA_MAX_RES], n_hel not in [1,PWA_MAX_HEL], n_chan not in [1,PWA_MAX_CHAN],
+ * res_chan out of range, n_events < 1, stride < n_events, mc.weight != NULL, misaligned borrowed
+ * buffers), uploads or adopts the event store, allocates scratch.  *out is NULL on failure. */
+pwa_status pwa_create(const pwa_model_desc* model, pwa_handle** out);
+pwa_status pwa_destroy(pwa_handle* h); /* NULL is allowed */
+int32_t pwa_n_params(const pwa_handle* h); /* 4*n_res, or -1 for NULL */
+
+/* ---- evaluation: device pointers, enqueue only ------------------------------------------------
+ * theta, v, grad, hv: P doubles; nll: 1 double.  PAPER.md:67 (Eq. 3), :90 (Eq. 6), :95 (Eq. 7). */
+pwa_status pwa_nll(pwa_handle* h, const double* theta, double* nll);
+pwa_status pwa_nll_grad(pwa_handle* h, const double* theta, double* nll, double* grad);
+pwa_status pwa_hvp(pwa_handle* h, const double* theta, const double* v, double* hv);
+/* the fused sweep: one streaming pass over all data and MC events gives all three */
+pwa_status pwa_nll_grad_hvp(pwa_handle* h, const double* theta, const double* v, double* nll,
+                            double* grad, double* hv);
+
+/* ---- shard interface (Eqs. 4-7) -----------------------------------------------
+ * pwa_raw_sums runs the same streaming pass but stops before the logarithm / division of Eqs. 4, 6, 7
+ * and writes the ADDITIVE raw sums of this handle's events:  raw[pwa_raw_size(h)] doubles (device)
+ *   raw[0] = sum_data w ln I   raw[1] = W = sum_data w   raw[2] = G = sum_mc I   raw[3] = N_mc
+ *   raw[4      .. 4+P)   gd = sum_data w g_i / I_i
+ *   raw[4+P    .. 4+2P)  gG = sum_mc g_j
+ *   raw[4+2P   .. 4+3P)  hd = sum_data w [ g_i (g_i.v)/I_i^2 - (H_i v)/I_i ]
+ *   raw[4+3P   .. 4+4P)  hG = sum_mc H_j v
+ * (g_i = grad_theta I_i, H_i = Hessian of I_i).  v may be NULL: the hd, hG blocks are then zero.
+ * Raw sums of disjoint shards add element-wise (that sum is the one all-reduce of a multi-GPU run);
+ * pwa_combine applies Eqs. 4, 6, 7 to the (summed) raw vector:
+ *   NLL = -raw[0] + W ln(G/N_mc);  grad = -gd + W gG/G;  Hv = hd + W [ hG/G - gG (gG.v)/G^2 ].
+ * nll, grad, hv may each be NULL (not wanted); hv requires v. */
+int32_t pwa_raw_size(const pwa_handle* h); /* 4 + 4P */
+pwa_status pwa_raw_sums(pwa_handle* h, const double* theta, const double* v, double* raw);
+pwa_status pwa_combine(pwa_handle* h, const double* raw, const double* v, double* nll, double* grad,
+                       double* hv);
+
+/* ---- fit ---------------------------------------------------------------------------------------
+ * Truncated line-search Newton-CG (Nocedal & Wright Alg. 7.1 as specialised in DESIGN.md (c-F);
+ * the paper names SciPy's Newton-CG, and gives no settings).  All vectors stay on the
+ * device; the host reads back a few scalars per iteration for control flow. */
+typedef struct {
+  int32_t max_outer;      /* 500   outer Newton iterations */
+  int32_t max_cg;         /* 50    CG iterations per outer step (BASELINE.json configs[4]) */
+  double gtol;            /* 1e-5  stop when |g|_inf <= gtol */
+  double xtol;            /* 1e-8  stop when t |p|_inf <= xtol */
+  double ftol;            /* 1e-12 stop when |f_new - f| <= ftol max(1,|f|) */
+  double armijo_c1;       /* 1e-4 */
+  double backtrack;       /* 0.5   step shrink factor rho */
+  int32_t max_backtrack;  /* 40 */
+  double max_seconds;     /* 0 = off; wall-time cap ("early stopping") */
+  double gamma_min, gamma_max, mass_min, mass_max; /* feasible box of the FIT only (S19): 5e-3, 2, 0.1, 4;
+                                                      a pair (0,0) switches that box off */
+  double gconv;           /* 1.0   a stopped fit counts as converged iff |g|_inf <= gconv */
+} pwa_fit_opts;
+
+typedef struct {
+  double nll;             /* NLL at the returned theta */
+  double grad_inf_norm;   /* |grad|_inf there */
+  int32_t outer_iters, cg_iters;
+  int32_t n_nll, n_grad, n_hvp; /* sweeps of each kind */
+  int32_t stop_reason;    /* 1 gtol, 2 xtol, 3 ftol, 4 max_outer, 5 max_seconds, 6 line search failed */
+  int32_t status;         /* PWA_OK (converged), PWA_ERR_NOT_CONVERGED or PWA_ERR_NONFINITE */
+  double seconds;         /* wall time of the call */
+} pwa_fit_result;
+
+void pwa_fit_opts_default(pwa_fit_opts* opts);
+/* theta_inout: DEVICE pointer, P doubles, start point in, final point out.  opts NULL = defaults.
+ * Returns result->status (or PWA_ERR_INVALID_ARG / PWA_ERR_CUDA).  Synchronises the stream. */
+pwa_status pwa_fit_newton_cg(pwa_handle* h, double* theta_inout, const pwa_fit_opts* opts,
+                             pwa_fit_result* result);
+
+/* ---- host-buffer convenience (the end-to-end path: copies in and out, synchronises) -------------
+ * theta_host, v_host: P doubles in HOST memory (v_host may be NULL: then grad_host only);
+ * nll_host 1 double, grad_host / hv_host P doubles in HOST memory (each may be NULL). */
+pwa_status pwa_nll_grad_hvp_host(pwa_handle* h, const double* theta_host, const double* v_host,
+                                 double* nll_host, double* grad_host, double* hv_host);
+
+/* ---- diagnostics -------------------------------------------------------------------------------*/
+/* Synchronises; *flags_host bit0 = the last evaluation produced a non-finite NLL, gradient or HVP. */
+pwa_status pwa_status_flags(pwa_handle* h, uint32_t* flags_host);
+/* Sweep-kernel timing for roofline reports: while enabled, the library brackets every sweep-kernel launch
+ * with a pair of CUDA events on the handle's stream (at most 4096 pairs are kept; later launches are not
+ * recorded).  pwa_profile_read synchronises the stream, returns the summed device time of the recorded
+ * sweep launches in milliseconds and their count, and clears the record.  Either output may be NULL. */
+pwa_status pwa_profile_enable(pwa_handle* h, int32_t on);
+pwa_status pwa_profile_read(pwa_handle* h, double* total_ms, int64_t* n_launches);
+/* Number of kernels this handle has launched since creation (never synchronises). */
+int64_t pwa_kernel_launches(const pwa_handle* h);
+/* Algorithmic HBM bytes one full evaluation reads: N_mc (16 R H + 8 C) + N_data (16 R H + 8 C [+8]). */
+int64_t pwa_bytes_per_eval(const pwa_handle* h);
+/* Name of the sweep-kernel variant the handle selected ("generic", ...), library-owned string. */
+const char* pwa_kernel_variant(const pwa_handle* h);
+/* Last error message of this handle (or of the last failed pwa_create if h is NULL). Library-owned. */
+const char* pwa_last_error(const pwa_handle* h);
+const char* pwa_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PWA_B200_H */

@@ -1,0 +1,337 @@
+"""Thin Python binding of libpwa_b200.so (include/pwa.h): argument marshalling only.
+
+Every step of the likelihood path runs in the library's CUDA kernels; PyTorch is used here for device
+memory (tensors whose data_ptr() is handed to the C ABI) and streams.  There is no CPU fallback: if
+the shared library is missing or no CUDA device is usable the calls raise.
+
+Function names mirror the C ABI: pwa_create, pwa_nll, pwa_nll_grad, pwa_hvp, pwa_nll_grad_hvp,
+pwa_raw_sums, pwa_combine, pwa_fit_newton_cg, pwa_nll_grad_hvp_host, ...
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, Structure, byref, c_char_p, c_double, c_int32, c_int64, c_uint32, c_void_p
+from typing import Optional
+
+__all__ = ["PwaError", "lib_path", "load", "pwa_create", "pwa_destroy", "pwa_n_params", "pwa_raw_size", "pwa_nll",
+           "pwa_nll_grad", "pwa_hvp", "pwa_nll_grad_hvp", "pwa_raw_sums", "pwa_combine", "pwa_fit_opts",
+           "pwa_fit_result", "pwa_fit_opts_default", "pwa_fit_newton_cg", "pwa_nll_grad_hvp_host",
+           "pwa_status_flags", "pwa_profile_enable", "pwa_profile_read", "pwa_kernel_launches", "pwa_bytes_per_eval",
+           "pwa_kernel_variant", "pwa_last_error", "pwa_version", "Model", "STATUS_NAMES", "EXPORTS"]
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB = None
+
+PWA_OK, PWA_ERR_INVALID_ARG, PWA_ERR_CUDA, PWA_ERR_OOM, PWA_ERR_NONFINITE, PWA_ERR_NOT_CONVERGED = range(6)
+STATUS_NAMES = ["PWA_OK", "PWA_ERR_INVALID_ARG", "PWA_ERR_CUDA", "PWA_ERR_OOM", "PWA_ERR_NONFINITE",
+                "PWA_ERR_NOT_CONVERGED"]
+PWA_MEM_HOST, PWA_MEM_DEVICE = 0, 1
+
+# every symbol include/pwa.h declares
+EXPORTS = ["pwa_create", "pwa_destroy", "pwa_n_params", "pwa_nll", "pwa_nll_grad", "pwa_hvp", "pwa_nll_grad_hvp",
+           "pwa_raw_size", "pwa_raw_sums", "pwa_combine", "pwa_fit_opts_default", "pwa_fit_newton_cg",
+           "pwa_nll_grad_hvp_host", "pwa_status_flags", "pwa_profile_enable", "pwa_profile_read",
+           "pwa_kernel_launches", "pwa_bytes_per_eval", "pwa_kernel_variant", "pwa_last_error", "pwa_version"]
+
+
+class PwaError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"{STATUS_NAMES[status] if 0 <= status < len(STATUS_NAMES) else status}: {msg}")
+        self.status = status
+
+
+class pwa_sample(Structure):
+    _fields_ = [("n_events", c_int64), ("stride", c_int64), ("mass", c_void_p), ("amp", c_void_p),
+                ("weight", c_void_p)]
+
+
+class pwa_model_desc(Structure):
+    _fields_ = [("n_res", c_int32), ("n_hel", c_int32), ("n_chan", c_int32), ("res_chan", c_void_p),
+                ("data", pwa_sample), ("mc", pwa_sample), ("mem", c_int32), ("borrow", c_int32),
+                ("device", c_int32), ("stream", c_void_p)]
+
+
+class pwa_fit_opts(Structure):
+    _fields_ = [("max_outer", c_int32), ("max_cg", c_int32), ("gtol", c_double), ("xtol", c_double),
+                ("ftol", c_double), ("armijo_c1", c_double), ("backtrack", c_double), ("max_backtrack", c_int32),
+                ("max_seconds", c_double), ("gamma_min", c_double), ("gamma_max", c_double),
+                ("mass_min", c_double), ("mass_max", c_double), ("gconv", c_double)]
+
+
+class pwa_fit_result(Structure):
+    _fields_ = [("nll", c_double), ("grad_inf_norm", c_double), ("outer_iters", c_int32), ("cg_iters", c_int32),
+                ("n_nll", c_int32), ("n_grad", c_int32), ("n_hvp", c_int32), ("stop_reason", c_int32),
+                ("status", c_int32), ("seconds", c_double)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+def lib_path() -> str:
+    return os.path.join(_HERE, "libpwa_b200.so")
+
+
+def load():
+    """Loads libpwa_b200.so (built by `python -m paper_2403_09225_b200.build`).  Raises if it is missing."""
+    global _LIB
+    if _LIB is not None:
+        return _LIB
+    path = lib_path()
+    if not os.path.exists(path):
+        raise RuntimeError(f"{path} is missing: build it with `python -m paper_2403_09225_b200.build` "
+                           "(there is no CPU fallback)")
+    lib = ctypes.CDLL(path)
+    vp, dp = c_void_p, c_void_p
+    lib.pwa_create.argtypes = [POINTER(pwa_model_desc), POINTER(vp)]
+    lib.pwa_destroy.argtypes = [vp]
+    lib.pwa_n_params.argtypes = [vp]
+    lib.pwa_raw_size.argtypes = [vp]
+    lib.pwa_nll.argtypes = [vp, dp, dp]
+    lib.pwa_nll_grad.argtypes = [vp, dp, dp, dp]
+    lib.pwa_hvp.argtypes = [vp, dp, dp, dp]
+    lib.pwa_nll_grad_hvp.argtypes = [vp, dp, dp, dp, dp, dp]
+    lib.pwa_raw_sums.argtypes = [vp, dp, dp, dp]
+    lib.pwa_combine.argtypes = [vp, dp, dp, dp, dp, dp]
+    lib.pwa_fit_opts_default.argtypes = [POINTER(pwa_fit_opts)]
+    lib.pwa_fit_opts_default.restype = None
+    lib.pwa_fit_newton_cg.argtypes = [vp, dp, POINTER(pwa_fit_opts), POINTER(pwa_fit_result)]
+    lib.pwa_nll_grad_hvp_host.argtypes = [vp, dp, dp, dp, dp, dp]
+    lib.pwa_status_flags.argtypes = [vp, POINTER(c_uint32)]
+    lib.pwa_profile_enable.argtypes = [vp, c_int32]
+    lib.pwa_profile_read.argtypes = [vp, POINTER(c_double), POINTER(c_int64)]
+    lib.pwa_kernel_launches.argtypes = [vp]
+    lib.pwa_kernel_launches.restype = c_int64
+    lib.pwa_bytes_per_eval.argtypes = [vp]
+    lib.pwa_bytes_per_eval.restype = c_int64
+    lib.pwa_kernel_variant.argtypes = [vp]
+    lib.pwa_kernel_variant.restype = c_char_p
+    lib.pwa_last_error.argtypes = [vp]
+    lib.pwa_last_error.restype = c_char_p
+    lib.pwa_version.argtypes = []
+    lib.pwa_version.restype = c_char_p
+    _LIB = lib
+    return lib
+
+
+def _check(status: int, h=None):
+    if status != PWA_OK:
+        raise PwaError(status, pwa_last_error(h))
+
+
+def _ptr(t) -> Optional[int]:
+    """Address of a torch tensor / numpy array / raw int, or None."""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    if hasattr(t, "data_ptr"):
+        return t.data_ptr()
+    return t.ctypes.data
+
+
+def _dev_f64(t, n, name):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+            and t.numel() >= n):
+        raise TypeError(f"{name}: expected a contiguous CUDA float64 tensor with >= {n} elements")
+    return t.data_ptr()
+
+
+# ---- the C calls, one to one ------------------------------------------------------------------------------
+def pwa_create(res_chan, data_mass, data_amp, data_weight, mc_mass, mc_amp, *, borrow: bool = False, device: int = 0,
+               stream: int = 0, data_stride: int = 0, mc_stride: int = 0, n_data: Optional[int] = None,
+               n_mc: Optional[int] = None) -> int:
+    """Creates a handle from torch tensors (CPU or CUDA, float64, contiguous) in the layouts of pwa.h:
+    mass [C][N], amp [R][H][N][2], weight [N] or None, res_chan [R] int32 (CPU).  Returns the handle."""
+    import torch
+    lib = load()
+    tensors = [data_mass, data_amp, mc_mass, mc_amp] + ([data_weight] if data_weight is not None else [])
+    on_dev = {t.is_cuda for t in tensors}
+    if len(on_dev) != 1:
+        raise TypeError("all event buffers must live on the same side (host or device)")
+    for t in tensors:
+        if t.dtype != torch.float64 or not t.is_contiguous():
+            raise TypeError("event buffers must be contiguous float64 tensors")
+    rc = res_chan.to(torch.int32).cpu().contiguous()
+    R, H = int(mc_amp.shape[0]), int(mc_amp.shape[1])
+    C = int(mc_mass.shape[0])
+    d = pwa_model_desc()
+    d.n_res, d.n_hel, d.n_chan = R, H, C
+    d.res_chan = rc.data_ptr()
+    d.data = pwa_sample(int(data_mass.shape[1]) if n_data is None else n_data, data_stride,
+                        data_mass.data_ptr(), data_amp.data_ptr(), _ptr(data_weight))
+    d.mc = pwa_sample(int(mc_mass.shape[1]) if n_mc is None else n_mc, mc_stride, mc_mass.data_ptr(),
+                      mc_amp.data_ptr(), None)
+    d.mem = PWA_MEM_DEVICE if on_dev.pop() else PWA_MEM_HOST
+    d.borrow = 1 if borrow else 0
+    d.device = device
+    d.stream = stream or None
+    out = c_void_p()
+    _check(lib.pwa_create(byref(d), byref(out)))
+    return out.value
+
+
+def pwa_destroy(h) -> None:
+    _check(load().pwa_destroy(h))
+
+
+def pwa_n_params(h) -> int:
+    return load().pwa_n_params(h)
+
+
+def pwa_raw_size(h) -> int:
+    return load().pwa_raw_size(h)
+
+
+def pwa_nll(h, theta, nll) -> None:
+    P = pwa_n_params(h)
+    _check(load().pwa_nll(h, _dev_f64(theta, P, "theta"), _dev_f64(nll, 1, "nll")), h)
+
+
+def pwa_nll_grad(h, theta, nll, grad) -> None:
+    P = pwa_n_params(h)
+    _check(load().pwa_nll_grad(h, _dev_f64(theta, P, "theta"), _dev_f64(nll, 1, "nll"), _dev_f64(grad, P, "grad")), h)
+
+
+def pwa_hvp(h, theta, v, hv) -> None:
+    P = pwa_n_params(h)
+    _check(load().pwa_hvp(h, _dev_f64(theta, P, "theta"), _dev_f64(v, P, "v"), _dev_f64(hv, P, "hv")), h)
+
+
+def pwa_nll_grad_hvp(h, theta, v, nll, grad, hv) -> None:
+    P = pwa_n_params(h)
+    _check(load().pwa_nll_grad_hvp(h, _dev_f64(theta, P, "theta"), _dev_f64(v, P, "v"), _dev_f64(nll, 1, "nll"),
+                                   _dev_f64(grad, P, "grad"), _dev_f64(hv, P, "hv")), h)
+
+
+def pwa_raw_sums(h, theta, v, raw) -> None:
+    P = pwa_n_params(h)
+    _check(load().pwa_raw_sums(h, _dev_f64(theta, P, "theta"), None if v is None else _dev_f64(v, P, "v"),
+                               _dev_f64(raw, 4 + 4 * P, "raw")), h)
+
+
+def pwa_combine(h, raw, v, nll, grad, hv) -> None:
+    P = pwa_n_params(h)
+    _check(load().pwa_combine(h, _dev_f64(raw, 4 + 4 * P, "raw"), None if v is None else _dev_f64(v, P, "v"),
+                              None if nll is None else _dev_f64(nll, 1, "nll"),
+                              None if grad is None else _dev_f64(grad, P, "grad"),
+                              None if hv is None else _dev_f64(hv, P, "hv")), h)
+
+
+def pwa_fit_opts_default() -> pwa_fit_opts:
+    o = pwa_fit_opts()
+    load().pwa_fit_opts_default(byref(o))
+    return o
+
+
+def pwa_fit_newton_cg(h, theta_inout, opts: Optional[pwa_fit_opts] = None) -> pwa_fit_result:
+    """Runs the fit; returns the result struct (status PWA_ERR_NOT_CONVERGED / NONFINITE are reported in
+    result.status, not raised); raises on argument or CUDA errors."""
+    P = pwa_n_params(h)
+    res = pwa_fit_result()
+    st = load().pwa_fit_newton_cg(h, _dev_f64(theta_inout, P, "theta"), byref(opts) if opts is not None else None,
+                                  byref(res))
+    if st in (PWA_ERR_INVALID_ARG, PWA_ERR_CUDA, PWA_ERR_OOM):
+        _check(st, h)
+    return res
+
+
+def pwa_nll_grad_hvp_host(h, theta_host, v_host, nll_host, grad_host, hv_host) -> None:
+    """Host-buffer entry point: numpy float64 arrays (or CPU tensors); copies in, evaluates, copies out, syncs."""
+    _check(load().pwa_nll_grad_hvp_host(h, _ptr(theta_host), _ptr(v_host), _ptr(nll_host), _ptr(grad_host),
+                                        _ptr(hv_host)), h)
+
+
+def pwa_status_flags(h) -> int:
+    f = c_uint32(0)
+    _check(load().pwa_status_flags(h, byref(f)), h)
+    return f.value
+
+
+def pwa_profile_enable(h, on: bool) -> None:
+    _check(load().pwa_profile_enable(h, 1 if on else 0), h)
+
+
+def pwa_profile_read(h):
+    """(summed sweep-kernel device time in ms, number of sweep launches) since the last read."""
+    ms, n = c_double(0.0), c_int64(0)
+    _check(load().pwa_profile_read(h, byref(ms), byref(n)), h)
+    return ms.value, n.value
+
+
+def pwa_kernel_launches(h) -> int:
+    return load().pwa_kernel_launches(h)
+
+
+def pwa_bytes_per_eval(h) -> int:
+    return load().pwa_bytes_per_eval(h)
+
+
+def pwa_kernel_variant(h) -> str:
+    return load().pwa_kernel_variant(h).decode()
+
+
+def pwa_last_error(h=None) -> str:
+    return load().pwa_last_error(h).decode()
+
+
+def pwa_version() -> str:
+    return load().pwa_version().decode()
+
+
+# ---- a small convenience wrapper (still marshalling only) ---------------------------------------------------
+class Model:
+    """Owns a handle and its output tensors.  `w` is a workloads.Workload (or any object with the same fields)."""
+
+    def __init__(self, w, device: int = 0, borrow: bool = False):
+        import torch
+        self.torch = torch
+        self.dev = torch.device("cuda", device)
+        self._keep = w if borrow else None
+        self.h = pwa_create(w.res_chan, w.data_mass, w.data_amp, w.data_weight, w.mc_mass, w.mc_amp, borrow=borrow,
+                            device=device)
+        self.P = pwa_n_params(self.h)
+        self.nll_t = torch.zeros(1, dtype=torch.float64, device=self.dev)
+        self.grad_t = torch.zeros(self.P, dtype=torch.float64, device=self.dev)
+        self.hv_t = torch.zeros(self.P, dtype=torch.float64, device=self.dev)
+
+    def _d(self, x):
+        return self.torch.as_tensor(x, dtype=self.torch.float64).to(self.dev).contiguous()
+
+    def nll(self, theta):
+        pwa_nll(self.h, self._d(theta), self.nll_t)
+        return self.nll_t.item()
+
+    def nll_grad(self, theta):
+        pwa_nll_grad(self.h, self._d(theta), self.nll_t, self.grad_t)
+        return self.nll_t.item(), self.grad_t.cpu().numpy().copy()
+
+    def hvp(self, theta, v):
+        pwa_hvp(self.h, self._d(theta), self._d(v), self.hv_t)
+        return self.hv_t.cpu().numpy().copy()
+
+    def nll_grad_hvp(self, theta, v):
+        pwa_nll_grad_hvp(self.h, self._d(theta), self._d(v), self.nll_t, self.grad_t, self.hv_t)
+        return self.nll_t.item(), self.grad_t.cpu().numpy().copy(), self.hv_t.cpu().numpy().copy()
+
+    def raw_sums(self, theta, v=None):
+        raw = self.torch.zeros(4 + 4 * self.P, dtype=self.torch.float64, device=self.dev)
+        pwa_raw_sums(self.h, self._d(theta), None if v is None else self._d(v), raw)
+        return raw
+
+    def fit(self, theta0, opts: Optional[pwa_fit_opts] = None):
+        th = self._d(theta0).clone()
+        res = pwa_fit_newton_cg(self.h, th, opts)
+        return th.cpu().numpy().copy(), res
+
+    def close(self):
+        if self.h:
+            pwa_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,424 @@
+// pwa_api.cu - the C ABI of include/pwa.h: handle, event store, evaluation entry points.
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <new>
+
+#include "pwa_internal.h"
+#include "pwa_kernels.cuh"
+
+namespace {
+std::mutex g_err_mutex;
+std::string g_create_err;
+
+void set_create_error(const std::string& s) {
+  std::lock_guard<std::mutex> lk(g_err_mutex);
+  g_create_err = s;
+}
+
+inline long long round_up(long long x, long long m) { return (x + m - 1) / m * m; }
+}  // namespace
+
+namespace pwa {
+
+pwa_status set_error(pwa_handle* h, pwa_status st, const char* what, cudaError_t ce) {
+  std::string msg = what ? what : "";
+  if (ce != cudaSuccess) {
+    msg += ": ";
+    msg += cudaGetErrorString(ce);
+  }
+  if (h) h->err = msg; else set_create_error(msg);
+  return st;
+}
+
+// ---- sweep dispatch -------------------------------------------------------------------------------
+typedef void (*sweep_fn)(const SweepArgs);
+
+template <int MODE>
+static sweep_fn generic_for_h(int H) {
+  switch (H) {
+    case 1: return k_sweep_generic<1, MODE>;
+    case 2: return k_sweep_generic<2, MODE>;
+    case 3: return k_sweep_generic<3, MODE>;
+    case 4: return k_sweep_generic<4, MODE>;
+    case 5: return k_sweep_generic<5, MODE>;
+    case 6: return k_sweep_generic<6, MODE>;
+    case 7: return k_sweep_generic<7, MODE>;
+    case 8: return k_sweep_generic<8, MODE>;
+  }
+  return nullptr;
+}
+
+static sweep_fn generic_fn(int H, int mode) {
+  switch (mode) {
+    case MODE_NLL: return generic_for_h<MODE_NLL>(H);
+    case MODE_GRAD: return generic_for_h<MODE_GRAD>(H);
+    default: return generic_for_h<MODE_FULL>(H);
+  }
+}
+
+static inline int nb_of(int R, int mode) {
+  if (mode == MODE_NLL) return 0;
+  const int rpb = rpb_of(mode);
+  return (R + rpb - 1) / rpb;
+}
+
+static size_t generic_smem(int block, int nb) { return (size_t)(block / 32) * ((size_t)nb * 32 + 2) * sizeof(double); }
+
+// Runs prologue + sweep + stage-2 reduction/unpack; leaves the public raw vector in `raw` (device).
+static pwa_status raw_sums_impl(pwa_handle* h, int mode, const double* theta, const double* v, double* raw) {
+  const int R = h->n_res;
+  if (mode == MODE_FULL && !v) mode = MODE_GRAD;
+  k_prologue<<<(R + 127) / 128, 128, 0, h->stream>>>(theta, mode == MODE_FULL ? v : nullptr, R, h->d_K);
+  h->launches++;
+  SweepArgs a;
+  a.s[0] = h->smp[0];
+  a.s[1] = h->smp[1];
+  a.K = h->d_K;
+  a.ch = h->d_ch;
+  a.R = R;
+  a.C = h->n_chan;
+  a.nb = nb_of(R, mode);
+  a.partial = h->d_partial;
+  sweep_fn fn = generic_fn(h->n_hel, mode);
+  const bool prof = h->profiling && h->prof_used + 2 <= h->prof_events.size();
+  if (prof) cudaEventRecord(h->prof_events[h->prof_used], h->stream);
+  fn<<<h->grid, h->block, generic_smem(h->block, a.nb), h->stream>>>(a);
+  h->launches++;
+  if (prof) {
+    cudaEventRecord(h->prof_events[h->prof_used + 1], h->stream);
+    h->prof_used += 2;
+  }
+  const double n_mc = (double)h->smp[0].n;
+  switch (mode) {
+    case MODE_NLL:
+      k_reduce_unpack<MODE_NLL><<<1, 1024, 0, h->stream>>>(h->d_partial, h->grid, a.nb, R, theta, v, n_mc, h->d_sums, raw);
+      break;
+    case MODE_GRAD:
+      k_reduce_unpack<MODE_GRAD><<<1, 1024, 0, h->stream>>>(h->d_partial, h->grid, a.nb, R, theta, v, n_mc, h->d_sums, raw);
+      break;
+    default:
+      k_reduce_unpack<MODE_FULL><<<1, 1024, 0, h->stream>>>(h->d_partial, h->grid, a.nb, R, theta, v, n_mc, h->d_sums, raw);
+      break;
+  }
+  h->launches++;
+  PWA_CUDA_CHECK(h, cudaGetLastError());
+  return PWA_OK;
+}
+
+static pwa_status combine_impl(pwa_handle* h, const double* raw, const double* v, double* nll, double* grad,
+                               double* hv) {
+  k_combine<<<1, 1024, 0, h->stream>>>(raw, v, h->n_par, nll, grad, hv, h->d_flags);
+  h->launches++;
+  PWA_CUDA_CHECK(h, cudaGetLastError());
+  return PWA_OK;
+}
+
+pwa_status eval(pwa_handle* h, int mode, const double* theta, const double* v, double* nll, double* grad, double* hv) {
+  pwa_status st = raw_sums_impl(h, mode, theta, v, h->d_raw);
+  if (st != PWA_OK) return st;
+  return combine_impl(h, h->d_raw, (mode == MODE_FULL) ? v : nullptr, nll, grad, (mode == MODE_FULL) ? hv : nullptr);
+}
+
+}  // namespace pwa
+
+using namespace pwa;
+
+// ---- creation -------------------------------------------------------------------------------------
+static pwa_status fail_create(pwa_handle* h, pwa_status st, const std::string& msg) {
+  set_create_error(msg);
+  if (h) pwa_destroy(h);
+  return st;
+}
+
+static bool validate_sample(const pwa_sample& s, const char* name, std::string& why) {
+  if (s.n_events < 1) { why = std::string(name) + ".n_events < 1"; return false; }
+  if (s.stride != 0 && s.stride < s.n_events) { why = std::string(name) + ".stride < n_events"; return false; }
+  if (!s.mass || !s.amp) { why = std::string(name) + ": null mass or amp"; return false; }
+  return true;
+}
+
+// Uploads or adopts one sample.  own[0..2] receive owned allocations (mass, amp, weight).
+static pwa_status store_sample(pwa_handle* h, const pwa_model_desc* m, const pwa_sample& s, int which, void** own) {
+  const long long n = s.n_events, sin = s.stride ? s.stride : s.n_events;
+  const int C = m->n_chan, planes = m->n_res * m->n_hel;
+  SampleDev& d = h->smp[which];
+  d.n = n;
+  if (m->mem == PWA_MEM_DEVICE && m->borrow) {
+    if (((uintptr_t)s.amp & 15) || ((uintptr_t)s.mass & 7) || (s.weight && ((uintptr_t)s.weight & 7)))
+      return set_error(nullptr, PWA_ERR_INVALID_ARG, "borrowed buffers are misaligned (amp 16 B, mass/weight 8 B)", cudaSuccess);
+    d.mass = s.mass;
+    d.amp = reinterpret_cast<const double2*>(s.amp);
+    d.weight = s.weight;
+    d.stride = sin;
+    return PWA_OK;
+  }
+  const long long so = round_up(n, 8);
+  d.stride = so;
+  const cudaMemcpyKind kind = m->mem == PWA_MEM_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  double *dm = nullptr, *da = nullptr, *dw = nullptr;
+  if (cudaMalloc(&dm, sizeof(double) * C * so) != cudaSuccess ||
+      cudaMalloc(&da, sizeof(double) * 2 * planes * so) != cudaSuccess ||
+      (s.weight && cudaMalloc(&dw, sizeof(double) * so) != cudaSuccess)) {
+    cudaGetLastError();
+    if (dm) cudaFree(dm);
+    if (da) cudaFree(da);
+    if (dw) cudaFree(dw);
+    return set_error(nullptr, PWA_ERR_OOM, "device allocation of the event store failed", cudaSuccess);
+  }
+  own[0] = dm; own[1] = da; own[2] = dw;
+  // zero the padding so that clamped tail lanes read defined values
+  PWA_CUDA_CHECK(nullptr, cudaMemsetAsync(dm, 0, sizeof(double) * C * so, h->stream));
+  PWA_CUDA_CHECK(nullptr, cudaMemsetAsync(da, 0, sizeof(double) * 2 * planes * so, h->stream));
+  for (int c = 0; c < C; ++c)
+    PWA_CUDA_CHECK(nullptr, cudaMemcpyAsync(dm + (size_t)c * so, s.mass + (size_t)c * sin, sizeof(double) * n, kind, h->stream));
+  for (int p = 0; p < planes; ++p)
+    PWA_CUDA_CHECK(nullptr, cudaMemcpyAsync(da + (size_t)p * so * 2, s.amp + (size_t)p * sin * 2, sizeof(double) * 2 * n, kind, h->stream));
+  if (s.weight) {
+    PWA_CUDA_CHECK(nullptr, cudaMemsetAsync(dw, 0, sizeof(double) * so, h->stream));
+    PWA_CUDA_CHECK(nullptr, cudaMemcpyAsync(dw, s.weight, sizeof(double) * n, kind, h->stream));
+  }
+  d.mass = dm;
+  d.amp = reinterpret_cast<const double2*>(da);
+  d.weight = dw;
+  return PWA_OK;
+}
+
+extern "C" pwa_status pwa_create(const pwa_model_desc* m, pwa_handle** out) {
+  if (out) *out = nullptr;
+  if (!m || !out) return fail_create(nullptr, PWA_ERR_INVALID_ARG, "null descriptor or output pointer");
+  if (m->n_res < 1 || m->n_res > PWA_MAX_RES) return fail_create(nullptr, PWA_ERR_INVALID_ARG, "n_res out of range");
+  if (m->n_hel < 1 || m->n_hel > PWA_MAX_HEL) return fail_create(nullptr, PWA_ERR_INVALID_ARG, "n_hel out of range");
+  if (m->n_chan < 1 || m->n_chan > PWA_MAX_CHAN) return fail_create(nullptr, PWA_ERR_INVALID_ARG, "n_chan out of range");
+  if (!m->res_chan) return fail_create(nullptr, PWA_ERR_INVALID_ARG, "null res_chan");
+  for (int r = 0; r < m->n_res; ++r)
+    if (m->res_chan[r] < 0 || m->res_chan[r] >= m->n_chan)
+      return fail_create(nullptr, PWA_ERR_INVALID_ARG, "res_chan value out of range");
+  std::string why;
+  if (!validate_sample(m->data, "data", why) || !validate_sample(m->mc, "mc", why))
+    return fail_create(nullptr, PWA_ERR_INVALID_ARG, why);
+  if (m->mc.weight) return fail_create(nullptr, PWA_ERR_INVALID_ARG, "mc.weight must be NULL (unweighted phase space)");
+  if (m->mem != PWA_MEM_HOST && m->mem != PWA_MEM_DEVICE) return fail_create(nullptr, PWA_ERR_INVALID_ARG, "bad mem kind");
+  if (m->borrow && m->mem != PWA_MEM_DEVICE) return fail_create(nullptr, PWA_ERR_INVALID_ARG, "borrow needs PWA_MEM_DEVICE");
+
+  int ndev = 0;
+  cudaError_t ce = cudaGetDeviceCount(&ndev);
+  if (ce != cudaSuccess || ndev < 1) {
+    cudaGetLastError();
+    return fail_create(nullptr, PWA_ERR_CUDA, std::string("no usable CUDA device: ") + cudaGetErrorString(ce));
+  }
+  if (m->device < 0 || m->device >= ndev) return fail_create(nullptr, PWA_ERR_INVALID_ARG, "device ordinal out of range");
+  if ((ce = cudaSetDevice(m->device)) != cudaSuccess)
+    return fail_create(nullptr, PWA_ERR_CUDA, std::string("cudaSetDevice: ") + cudaGetErrorString(ce));
+
+  pwa_handle* h = new (std::nothrow) pwa_handle();
+  if (!h) return fail_create(nullptr, PWA_ERR_OOM, "host allocation failed");
+  h->device = m->device;
+  h->stream = static_cast<cudaStream_t>(m->stream);
+  h->n_res = m->n_res;
+  h->n_hel = m->n_hel;
+  h->n_chan = m->n_chan;
+  h->n_par = 4 * m->n_res;
+  h->weighted = m->data.weight != nullptr;
+  cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, m->device);
+
+  pwa_status st = store_sample(h, m, m->mc, 0, h->owned);
+  if (st == PWA_OK) st = store_sample(h, m, m->data, 1, h->owned + 3);
+  if (st != PWA_OK) {
+    std::string msg;
+    { std::lock_guard<std::mutex> lk(g_err_mutex); msg = g_create_err; }
+    return fail_create(h, st, msg);
+  }
+
+  // ---- launch configuration of the sweep (fixed for the life of the handle) ------------------------
+  const int R = h->n_res, P = h->n_par;
+  const int nb_full = nb_of(R, MODE_FULL);
+  int block = 256;
+  while (block > 32 && generic_smem(block, nb_full) > 160 * 1024) block /= 2;
+  const size_t smem = generic_smem(block, nb_full);
+  int occ_min = 1 << 30;
+  for (int mode = 0; mode < 3; ++mode) {
+    sweep_fn fn = generic_fn(h->n_hel, mode);
+    if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess)
+      return fail_create(h, PWA_ERR_CUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(ce));
+    int occ = 0;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, block, generic_smem(block, nb_of(R, mode)));
+    if (occ < 1) occ = 1;
+    if (occ < occ_min) occ_min = occ;
+  }
+  h->block = block;
+  h->grid = h->num_sms * occ_min;
+  h->variant_name = "generic";
+
+  const size_t pstride = (size_t)nb_full * 32 + 2;
+  h->partial_doubles = 2 * (size_t)h->grid * pstride;
+  const size_t io = 1 + 4 * (size_t)P + 8;
+  bool ok = cudaMalloc(&h->d_ch, sizeof(int) * R) == cudaSuccess &&
+            cudaMalloc(&h->d_K, sizeof(double) * KSTRIDE * R) == cudaSuccess &&
+            cudaMalloc(&h->d_partial, sizeof(double) * h->partial_doubles) == cudaSuccess &&
+            cudaMalloc(&h->d_sums, sizeof(double) * 2 * pstride) == cudaSuccess &&
+            cudaMalloc(&h->d_raw, sizeof(double) * (4 + 4 * (size_t)P)) == cudaSuccess &&
+            cudaMalloc(&h->d_flags, sizeof(unsigned)) == cudaSuccess &&
+            cudaMalloc(&h->d_io, sizeof(double) * io) == cudaSuccess &&
+            cudaMalloc(&h->d_fit, sizeof(double) * (8 * (size_t)P + 64)) == cudaSuccess &&
+            cudaMallocHost(&h->h_pin, sizeof(double) * io) == cudaSuccess &&
+            cudaMallocHost(&h->h_fit, sizeof(double) * 64) == cudaSuccess;
+  if (!ok) {
+    cudaGetLastError();
+    return fail_create(h, PWA_ERR_OOM, "scratch allocation failed");
+  }
+  if ((ce = cudaMemcpyAsync(h->d_ch, m->res_chan, sizeof(int) * R, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
+      (ce = cudaMemsetAsync(h->d_flags, 0, sizeof(unsigned), h->stream)) != cudaSuccess ||
+      (ce = cudaStreamSynchronize(h->stream)) != cudaSuccess)
+    return fail_create(h, PWA_ERR_CUDA, std::string("upload: ") + cudaGetErrorString(ce));
+  *out = h;
+  return PWA_OK;
+}
+
+extern "C" pwa_status pwa_destroy(pwa_handle* h) {
+  if (!h) return PWA_OK;
+  cudaSetDevice(h->device);
+  cudaStreamSynchronize(h->stream);
+  for (void* p : h->owned) if (p) cudaFree(p);
+  void* dev[] = {h->d_ch, h->d_K, h->d_partial, h->d_sums, h->d_raw, h->d_flags, h->d_io, h->d_fit};
+  for (void* p : dev) if (p) cudaFree(p);
+  for (cudaEvent_t e : h->prof_events) cudaEventDestroy(e);
+  if (h->h_pin) cudaFreeHost(h->h_pin);
+  if (h->h_fit) cudaFreeHost(h->h_fit);
+  cudaGetLastError();
+  delete h;
+  return PWA_OK;
+}
+
+extern "C" int32_t pwa_n_params(const pwa_handle* h) { return h ? h->n_par : -1; }
+extern "C" int32_t pwa_raw_size(const pwa_handle* h) { return h ? 4 + 4 * h->n_par : -1; }
+
+// ---- evaluation -------------------------------------------------------------------------------------
+#define PWA_REQUIRE(h, cond, msg) \
+  do { if (!(cond)) return pwa::set_error((h), PWA_ERR_INVALID_ARG, msg, cudaSuccess); } while (0)
+
+extern "C" pwa_status pwa_nll(pwa_handle* h, const double* theta, double* nll) {
+  if (!h) return PWA_ERR_INVALID_ARG;
+  PWA_REQUIRE(h, theta && nll, "pwa_nll: null pointer");
+  return eval(h, MODE_NLL, theta, nullptr, nll, nullptr, nullptr);
+}
+
+extern "C" pwa_status pwa_nll_grad(pwa_handle* h, const double* theta, double* nll, double* grad) {
+  if (!h) return PWA_ERR_INVALID_ARG;
+  PWA_REQUIRE(h, theta && nll && grad, "pwa_nll_grad: null pointer");
+  return eval(h, MODE_GRAD, theta, nullptr, nll, grad, nullptr);
+}
+
+extern "C" pwa_status pwa_hvp(pwa_handle* h, const double* theta, const double* v, double* hv) {
+  if (!h) return PWA_ERR_INVALID_ARG;
+  PWA_REQUIRE(h, theta && v && hv, "pwa_hvp: null pointer");
+  return eval(h, MODE_FULL, theta, v, nullptr, nullptr, hv);
+}
+
+extern "C" pwa_status pwa_nll_grad_hvp(pwa_handle* h, const double* theta, const double* v, double* nll, double* grad,
+                                       double* hv) {
+  if (!h) return PWA_ERR_INVALID_ARG;
+  PWA_REQUIRE(h, theta && v && nll && grad && hv, "pwa_nll_grad_hvp: null pointer");
+  return eval(h, MODE_FULL, theta, v, nll, grad, hv);
+}
+
+extern "C" pwa_status pwa_raw_sums(pwa_handle* h, const double* theta, const double* v, double* raw) {
+  if (!h) return PWA_ERR_INVALID_ARG;
+  PWA_REQUIRE(h, theta && raw, "pwa_raw_sums: null pointer");
+  return raw_sums_impl(h, v ? MODE_FULL : MODE_GRAD, theta, v, raw);
+}
+
+extern "C" pwa_status pwa_combine(pwa_handle* h, const double* raw, const double* v, double* nll, double* grad,
+                                  double* hv) {
+  if (!h) return PWA_ERR_INVALID_ARG;
+  PWA_REQUIRE(h, raw, "pwa_combine: null raw");
+  PWA_REQUIRE(h, !hv || v, "pwa_combine: hv requires v");
+  return combine_impl(h, raw, v, nll, grad, hv);
+}
+
+extern "C" pwa_status pwa_nll_grad_hvp_host(pwa_handle* h, const double* theta_host, const double* v_host,
+                                            double* nll_host, double* grad_host, double* hv_host) {
+  if (!h) return PWA_ERR_INVALID_ARG;
+  PWA_REQUIRE(h, theta_host, "pwa_nll_grad_hvp_host: null theta");
+  PWA_REQUIRE(h, !hv_host || v_host, "pwa_nll_grad_hvp_host: hv requires v");
+  const size_t P = h->n_par;
+  double* d_theta = h->d_io;
+  double* d_v = h->d_io + P;
+  double* d_out = h->d_io + 2 * P;  // nll | grad | hv
+  std::memcpy(h->h_pin, theta_host, sizeof(double) * P);
+  if (v_host) std::memcpy(h->h_pin + P, v_host, sizeof(double) * P);
+  PWA_CUDA_CHECK(h, cudaMemcpyAsync(d_theta, h->h_pin, sizeof(double) * (v_host ? 2 * P : P), cudaMemcpyHostToDevice, h->stream));
+  pwa_status st = eval(h, v_host ? MODE_FULL : MODE_GRAD, d_theta, v_host ? d_v : nullptr, d_out, d_out + 1,
+                       v_host ? d_out + 1 + P : nullptr);
+  if (st != PWA_OK) return st;
+  const size_t nout = 1 + P + (v_host ? P : 0);
+  PWA_CUDA_CHECK(h, cudaMemcpyAsync(h->h_pin + 2 * P, d_out, sizeof(double) * nout, cudaMemcpyDeviceToHost, h->stream));
+  PWA_CUDA_CHECK(h, cudaStreamSynchronize(h->stream));
+  if (nll_host) *nll_host = h->h_pin[2 * P];
+  if (grad_host) std::memcpy(grad_host, h->h_pin + 2 * P + 1, sizeof(double) * P);
+  if (hv_host) std::memcpy(hv_host, h->h_pin + 2 * P + 1 + P, sizeof(double) * P);
+  return PWA_OK;
+}
+
+// ---- diagnostics --------------------------------------------------------------------------------------
+extern "C" pwa_status pwa_status_flags(pwa_handle* h, uint32_t* flags_host) {
+  if (!h) return PWA_ERR_INVALID_ARG;
+  PWA_REQUIRE(h, flags_host, "pwa_status_flags: null pointer");
+  unsigned f = 0;
+  PWA_CUDA_CHECK(h, cudaMemcpyAsync(&f, h->d_flags, sizeof(unsigned), cudaMemcpyDeviceToHost, h->stream));
+  PWA_CUDA_CHECK(h, cudaStreamSynchronize(h->stream));
+  *flags_host = f;
+  return PWA_OK;
+}
+
+extern "C" pwa_status pwa_profile_enable(pwa_handle* h, int32_t on) {
+  if (!h) return PWA_ERR_INVALID_ARG;
+  if (on && h->prof_events.empty()) {
+    h->prof_events.resize(2 * 4096);
+    for (size_t i = 0; i < h->prof_events.size(); ++i) {
+      cudaError_t ce = cudaEventCreate(&h->prof_events[i]);
+      if (ce != cudaSuccess) {
+        for (size_t j = 0; j < i; ++j) cudaEventDestroy(h->prof_events[j]);
+        h->prof_events.clear();
+        return pwa::set_error(h, PWA_ERR_CUDA, "cudaEventCreate", ce);
+      }
+    }
+  }
+  h->profiling = on != 0;
+  return PWA_OK;
+}
+
+extern "C" pwa_status pwa_profile_read(pwa_handle* h, double* total_ms, int64_t* n_launches) {
+  if (!h) return PWA_ERR_INVALID_ARG;
+  PWA_CUDA_CHECK(h, cudaStreamSynchronize(h->stream));
+  double tot = 0.0;
+  for (size_t i = 0; i + 1 < h->prof_used; i += 2) {
+    float ms = 0.f;
+    PWA_CUDA_CHECK(h, cudaEventElapsedTime(&ms, h->prof_events[i], h->prof_events[i + 1]));
+    tot += ms;
+  }
+  if (total_ms) *total_ms = tot;
+  if (n_launches) *n_launches = (int64_t)(h->prof_used / 2);
+  h->prof_used = 0;
+  return PWA_OK;
+}
+
+extern "C" int64_t pwa_kernel_launches(const pwa_handle* h) { return h ? h->launches : -1; }
+
+extern "C" int64_t pwa_bytes_per_eval(const pwa_handle* h) {
+  if (!h) return -1;
+  const long long per = 16LL * h->n_res * h->n_hel + 8LL * h->n_chan;
+  return h->smp[0].n * per + h->smp[1].n * (per + (h->weighted ? 8 : 0));
+}
+
+extern "C" const char* pwa_kernel_variant(const pwa_handle* h) { return h ? h->variant_name : ""; }
+
+extern "C" const char* pwa_last_error(const pwa_handle* h) {
+  if (h) return h->err.c_str();
+  static thread_local std::string copy;
+  std::lock_guard<std::mutex> lk(g_err_mutex);
+  copy = g_create_err;
+  return copy.c_str();
+}
+
+extern "C" const char* pwa_version(void) { return "pwa-b200 0.1 (sm_100a)"; }

@@ -1,0 +1,60 @@
+// pwa_internal.h - host-side handle layout shared by pwa_api.cu and pwa_fit.cu (not installed).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/pwa.h"
+#include "pwa_common.cuh"
+
+struct pwa_handle {
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  int n_res = 0, n_hel = 0, n_chan = 0, n_par = 0;
+  int num_sms = 0;
+  bool weighted = false;
+
+  // event store (a-0): device pointers, owned unless borrowed
+  pwa::SampleDev smp[2];  // 0 = MC, 1 = data
+  void* owned[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  int* d_ch = nullptr;
+
+  // scratch
+  double* d_K = nullptr;        // per-resonance constants
+  double* d_partial = nullptr;  // per-block partial sums
+  double* d_sums = nullptr;     // block-summed compact sums
+  double* d_raw = nullptr;      // public raw vector (4 + 4P)
+  unsigned* d_flags = nullptr;
+  size_t partial_doubles = 0;
+
+  // sweep launch configuration (fixed at creation -> deterministic event -> thread map)
+  int grid = 0, block = 0;
+  int variant = 0;
+  const char* variant_name = "generic";
+
+  // device staging for the *_host entry point and the fit driver
+  double* d_io = nullptr;   // theta | v | nll | grad | hv   (1 + 4P doubles, padded)
+  double* h_pin = nullptr;  // pinned host mirror of d_io
+  double* d_fit = nullptr;  // fit vectors
+  double* h_fit = nullptr;  // pinned scalars of the fit driver
+
+  long long launches = 0;
+  bool profiling = false;
+  std::vector<cudaEvent_t> prof_events;  // pairs (start, stop)
+  size_t prof_used = 0;
+  std::string err;
+};
+
+namespace pwa {
+// internal entry points used by the fit driver (enqueue only)
+pwa_status eval(pwa_handle* h, int mode, const double* theta, const double* v, double* nll, double* grad,
+                double* hv);
+pwa_status set_error(pwa_handle* h, pwa_status st, const char* what, cudaError_t ce);
+}  // namespace pwa
+
+#define PWA_CUDA_CHECK(h, call)                                              \
+  do {                                                                       \
+    cudaError_t ce__ = (call);                                               \
+    if (ce__ != cudaSuccess) return pwa::set_error((h), PWA_ERR_CUDA, #call, ce__); \
+  } while (0)

@@ -1,0 +1,169 @@
+"""GPU parity: the CUDA path (through the C ABI of include/pwa.h) against the CPU oracle, element by
+element on the same seeded inputs.  Tolerances are BASELINE.json's north_star: NLL 1e-10 relative,
+gradient and HVP 1e-8 relative L2 (denominators: DESIGN.md S12); repeat runs bit-identical.
+
+Sizes: BASELINE.json config shapes scaled to what the 80-bit oracle finishes in seconds, always with a
+ragged tail (event counts that are not multiples of 32 or of any tile size).
+"""
+import numpy as np
+import pytest
+import torch
+
+from helpers import rel_l2
+
+pytestmark = pytest.mark.gpu
+
+NLL_TOL = 1e-10
+VEC_TOL = 1e-8
+
+# (config index, n_mc, n_data): config shapes of BASELINE.json at oracle-sized event counts
+CASES = [(1, 50_000, 10_000), (2, 20_011, 3_001), (3, 12_345, 1_537), (4, 2_049, 517), (6, 30_001, 1_999)]
+
+
+@pytest.fixture(scope="module")
+def pwa():
+    import paper_2403_09225_b200 as p
+    from paper_2403_09225_b200.build import build
+    build()
+    p.load()
+    assert torch.cuda.is_available(), "the gpu tests need a CUDA device"
+    return p
+
+
+_CACHE = {}
+
+
+def _case(pwa, oracle_mod, idx, n_mc, n_data):
+    key = (idx, n_mc, n_data)
+    if key not in _CACHE:
+        import workloads
+        cfg = workloads.CONFIGS[idx].scaled(n_mc, n_data)
+        w = workloads.make_workload(cfg, "cpu", chunk=1 << 13)
+        om = oracle_mod.model_from_workload(w)
+        gm = pwa.Model(w)
+        _CACHE[key] = (cfg, w, om, gm)
+    return _CACHE[key]
+
+
+def _thetas(cfg):
+    import workloads
+    return [workloads.theta_true(cfg).numpy()] + [workloads.random_start(cfg, k).numpy() for k in range(3)]
+
+
+def _nll_err(a, b):
+    return abs(float(a) - float(b)) / max(abs(float(b)), 1.0)
+
+
+@pytest.mark.parametrize("idx,n_mc,n_data", CASES)
+def test_fused_sweep_matches_oracle(pwa, oracle_mod, idx, n_mc, n_data):
+    import workloads
+    cfg, w, om, gm = _case(pwa, oracle_mod, idx, n_mc, n_data)
+    for k, th in enumerate(_thetas(cfg)):
+        v = workloads.direction(cfg, k).numpy()
+        f0, g0, h0 = oracle_mod.nll_grad_hvp(om, th, v, "ld")
+        f, g, hv = gm.nll_grad_hvp(th, v)
+        assert _nll_err(f, f0) < NLL_TOL, (idx, k, f, float(f0))
+        assert rel_l2(g, g0) < VEC_TOL, (idx, k)
+        assert rel_l2(hv, h0) < VEC_TOL, (idx, k)
+        assert pwa.pwa_status_flags(gm.h) == 0
+
+
+@pytest.mark.parametrize("idx,n_mc,n_data", CASES[:4])
+def test_separate_calls_match_oracle(pwa, oracle_mod, idx, n_mc, n_data):
+    import workloads
+    cfg, w, om, gm = _case(pwa, oracle_mod, idx, n_mc, n_data)
+    th = _thetas(cfg)[1]
+    v = workloads.direction(cfg, 5).numpy()
+    f0, g0, h0 = oracle_mod.nll_grad_hvp(om, th, v, "ld")
+    assert _nll_err(gm.nll(th), f0) < NLL_TOL
+    f, g = gm.nll_grad(th)
+    assert _nll_err(f, f0) < NLL_TOL and rel_l2(g, g0) < VEC_TOL
+    assert rel_l2(gm.hvp(th, v), h0) < VEC_TOL
+
+
+@pytest.mark.parametrize("idx,n_mc,n_data", CASES[:3])
+def test_repeat_runs_are_bit_identical(pwa, oracle_mod, idx, n_mc, n_data):
+    import workloads
+    cfg, w, om, gm = _case(pwa, oracle_mod, idx, n_mc, n_data)
+    th, v = _thetas(cfg)[0], workloads.direction(cfg, 0).numpy()
+    a = gm.nll_grad_hvp(th, v)
+    for _ in range(3):
+        b = gm.nll_grad_hvp(th, v)
+        assert np.float64(a[0]).tobytes() == np.float64(b[0]).tobytes()
+        assert a[1].tobytes() == b[1].tobytes() and a[2].tobytes() == b[2].tobytes()
+    # a second handle on the same arrays gives the same bits too
+    gm2 = pwa.Model(w)
+    c = gm2.nll_grad_hvp(th, v)
+    assert a[1].tobytes() == c[1].tobytes() and a[2].tobytes() == c[2].tobytes()
+    gm2.close()
+
+
+def test_invariance_directions_on_device(pwa, oracle_mod):
+    """Global phase: H 1_phi = 0, g.1_phi = 0; common scale: g.u = 0, (H u)_a = -g_a (P2)."""
+    cfg, w, om, gm = _case(pwa, oracle_mod, *CASES[1])
+    th = _thetas(cfg)[2]
+    P = cfg.n_par
+    ones_phi = np.zeros(P); ones_phi[1::4] = 1.0
+    u = np.zeros(P); u[0::4] = th[0::4]
+    f, g, h1 = gm.nll_grad_hvp(th, ones_phi)
+    scale = np.linalg.norm(gm.hvp(th, np.ones(P)))
+    assert np.linalg.norm(h1) < 1e-9 * scale
+    assert abs(g @ ones_phi) < 1e-9 * np.linalg.norm(g) * np.sqrt(P)
+    assert abs(g @ u) < 1e-9 * np.linalg.norm(g) * np.linalg.norm(u)
+    hu = gm.hvp(th, u)
+    assert np.linalg.norm(hu[0::4] + g[0::4]) < 1e-8 * max(np.linalg.norm(g[0::4]), 1e-300) + 1e-9 * scale
+    # the oracle agrees on those special directions as well
+    _, _, h0 = oracle_mod.nll_grad_hvp(om, th, u, "ld")
+    assert rel_l2(hu, h0) < VEC_TOL
+
+
+def test_shard_additivity_through_raw_sums(pwa, oracle_mod):
+    """PAPER.md:80-96 (Eqs. 4-7): raw sums of two disjoint shards add to the raw sums of the whole."""
+    import workloads
+    cfg, w, om, gm = _case(pwa, oracle_mod, *CASES[2])
+    th, v = _thetas(cfg)[1], workloads.direction(cfg, 1).numpy()
+    nm, nd = cfg.n_mc, cfg.n_data
+    cut_m, cut_d = 5_003, 700
+    parts = []
+    for (m0, m1, d0, d1) in ((0, cut_m, 0, cut_d), (cut_m, nm, cut_d, nd)):
+        h = pwa.pwa_create(w.res_chan, w.data_mass[:, d0:d1].contiguous(), w.data_amp[:, :, d0:d1].contiguous(),
+                           None if w.data_weight is None else w.data_weight[d0:d1].contiguous(),
+                           w.mc_mass[:, m0:m1].contiguous(), w.mc_amp[:, :, m0:m1].contiguous())
+        raw = torch.zeros(pwa.pwa_raw_size(h), dtype=torch.float64, device="cuda")
+        pwa.pwa_raw_sums(h, torch.tensor(th, device="cuda"), torch.tensor(v, device="cuda"), raw)
+        parts.append(raw.clone())
+        torch.cuda.synchronize()
+        pwa.pwa_destroy(h)
+    total = parts[0] + parts[1]
+    whole = gm.raw_sums(th, v)
+    assert float(total[3]) == nm and float(whole[3]) == nm
+    assert rel_l2(total.cpu().numpy(), whole.cpu().numpy()) < 1e-13
+    nll = torch.zeros(1, dtype=torch.float64, device="cuda")
+    g = torch.zeros(cfg.n_par, dtype=torch.float64, device="cuda")
+    hv = torch.zeros(cfg.n_par, dtype=torch.float64, device="cuda")
+    pwa.pwa_combine(gm.h, total, torch.tensor(v, device="cuda"), nll, g, hv)
+    f0, g0, h0 = oracle_mod.nll_grad_hvp(om, th, v, "ld")
+    assert _nll_err(nll.item(), f0) < NLL_TOL
+    assert rel_l2(g.cpu().numpy(), g0) < VEC_TOL and rel_l2(hv.cpu().numpy(), h0) < VEC_TOL
+    # and the raw vector itself matches the oracle's raw sums block by block
+    sd, gd, hd = oracle_mod.raw_sums(om, "data", th, v, "ld")
+    sm, gG, hG = oracle_mod.raw_sums(om, "mc", th, v, "ld")
+    P = cfg.n_par
+    wh = whole.cpu().numpy()
+    assert _nll_err(wh[0], sd[0]) < NLL_TOL and _nll_err(wh[1], sd[1]) < 1e-13 and _nll_err(wh[2], sm[0]) < 1e-12
+    for k, ref in enumerate((gd, gG, hd, hG)):
+        assert rel_l2(wh[4 + k * P: 4 + (k + 1) * P], ref) < VEC_TOL, k
+
+
+def test_host_entry_point(pwa, oracle_mod):
+    import workloads
+    cfg, w, om, gm = _case(pwa, oracle_mod, *CASES[1])
+    th, v = _thetas(cfg)[0], workloads.direction(cfg, 2).numpy()
+    nll = np.zeros(1); g = np.zeros(cfg.n_par); hv = np.zeros(cfg.n_par)
+    pwa.pwa_nll_grad_hvp_host(gm.h, np.ascontiguousarray(th), np.ascontiguousarray(v), nll, g, hv)
+    f1, g1, h1 = gm.nll_grad_hvp(th, v)
+    assert nll[0] == f1 and g.tobytes() == g1.tobytes() and hv.tobytes() == h1.tobytes()
+    g2 = np.zeros(cfg.n_par)
+    pwa.pwa_nll_grad_hvp_host(gm.h, np.ascontiguousarray(th), None, nll, g2, None)
+    f0, g0, _ = oracle_mod.nll_grad_hvp(om, th, None, "ld")
+    assert _nll_err(nll[0], f0) < NLL_TOL and rel_l2(g2, g0) < VEC_TOL
