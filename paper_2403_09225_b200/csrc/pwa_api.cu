@@ -71,6 +71,7 @@ static pwa_status raw_sums_impl(pwa_handle* h, int mode, const double* theta, co
   if (mode == MODE_FULL && !v) mode = MODE_GRAD;
   k_prologue<<<(R + 127) / 128, 128, 0, h->stream>>>(theta, mode == MODE_FULL ? v : nullptr, R, h->d_K);
   h->launches++;
+  if (cudaError_t ce = cudaGetLastError()) return set_error(h, PWA_ERR_CUDA, "launch k_prologue", ce);
   SweepArgs a;
   a.s[0] = h->smp[0];
   a.s[1] = h->smp[1];
@@ -89,6 +90,7 @@ static pwa_status raw_sums_impl(pwa_handle* h, int mode, const double* theta, co
     cudaEventRecord(h->prof_events[h->prof_used + 1], h->stream);
     h->prof_used += 2;
   }
+  if (cudaError_t ce = cudaGetLastError()) return set_error(h, PWA_ERR_CUDA, "launch sweep kernel", ce);
   const double n_mc = (double)h->smp[0].n;
   switch (mode) {
     case MODE_NLL:
@@ -102,7 +104,7 @@ static pwa_status raw_sums_impl(pwa_handle* h, int mode, const double* theta, co
       break;
   }
   h->launches++;
-  PWA_CUDA_CHECK(h, cudaGetLastError());
+  if (cudaError_t ce = cudaGetLastError()) return set_error(h, PWA_ERR_CUDA, "launch k_reduce_unpack", ce);
   return PWA_OK;
 }
 
@@ -110,7 +112,7 @@ static pwa_status combine_impl(pwa_handle* h, const double* raw, const double* v
                                double* hv) {
   k_combine<<<1, 1024, 0, h->stream>>>(raw, v, h->n_par, nll, grad, hv, h->d_flags);
   h->launches++;
-  PWA_CUDA_CHECK(h, cudaGetLastError());
+  if (cudaError_t ce = cudaGetLastError()) return set_error(h, PWA_ERR_CUDA, "launch k_combine", ce);
   return PWA_OK;
 }
 
@@ -235,7 +237,8 @@ extern "C" pwa_status pwa_create(const pwa_model_desc* m, pwa_handle** out) {
   const int nb_full = nb_of(R, MODE_FULL);
   int block = 256;
   while (block > 32 && generic_smem(block, nb_full) > 160 * 1024) block /= 2;
-  const size_t smem = generic_smem(block, nb_full);
+  // the opt-in limit is a property of the function, shared by every handle: always raise it to one fixed cap
+  const size_t smem = 200 * 1024;
   int occ_min = 1 << 30;
   for (int mode = 0; mode < 3; ++mode) {
     sweep_fn fn = generic_fn(h->n_hel, mode);
