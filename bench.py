@@ -1,0 +1,313 @@
+#!/usr/bin/env python
+"""bench.py - the NLL + gradient + HVP sweep of BASELINE.json's target configuration on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
+
+One "step" = one pwa_nll_grad_hvp call = one streaming pass of the whole hot path (propagators, coherent
+and incoherent sums, ln I, NLL, gradient, HVP, reduction, Eqs. 4/6/7) over all MC and data events of the
+workload.  Prints ONE JSON line (rank 0).  See DESIGN.md §Measurement for every field.
+
+N > 1 (launched with torch.distributed.run): weak scaling over event shards as in PAPER.md:78-98 - every
+rank holds its own config-sized shard, runs pwa_raw_sums on it, the raw vectors (4 + 4P doubles) are
+all-reduced with NCCL and every rank applies pwa_combine (Eqs. 4, 6, 7).
+
+--impl reference times the CPU oracle (oracle/, test infrastructure) on a bounded sample of the same
+workload on this box's host cores; it is a deliberately plain program, not a target.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "nll_grad_hvp_events_per_s"
+UNIT = "events/s"
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return float(p["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc, self.thread = index, [], None, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        inside = [r for (t, r) in self.rows if t0 <= t <= t1] or [r for (_, r) in self.rows[-3:]]
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in inside:
+            f = [x.strip() for x in r.split(",")]
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except (ValueError, IndexError):
+                continue
+            for n, val in zip(names, f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(n)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def _oracle_sample_time(w, n_mc_s, n_data_s, th, v, threads):
+    """Times the CPU oracle (double build, OpenMP) on the first n_mc_s / n_data_s events of the workload."""
+    import oracle
+    import numpy as np
+    to_np = lambda t: None if t is None else t.detach().cpu().numpy()
+    data = oracle.Sample(to_np(w.data_mass[:, :n_data_s]), to_np(w.data_amp[:, :, :n_data_s]),
+                         to_np(None if w.data_weight is None else w.data_weight[:n_data_s]))
+    mc = oracle.Sample(to_np(w.mc_mass[:, :n_mc_s]), to_np(w.mc_amp[:, :, :n_mc_s]), None)
+    m = oracle.Model(to_np(w.res_chan), data, mc)
+    t0 = time.perf_counter()
+    out = oracle.nll_grad_hvp(m, np.asarray(th), np.asarray(v), "d", threads=threads)
+    return time.perf_counter() - t0, out
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands, on host cores, on a bounded sample of the workload per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import torch
+    import oracle
+    import workloads
+    oracle.build()
+    cfg = workloads.CONFIGS[args.config]
+    # bounded sample: same model (R, H, C, weights), fewer events, same MC:data ratio
+    n_mc_s = min(cfg.n_mc, args.ref_events)
+    n_data_s = max(1, n_mc_s * cfg.n_data // cfg.n_mc)
+    dev = "cuda" if torch.cuda.is_available() else "cpu"
+    w = workloads.make_workload(cfg.scaled(n_mc_s, n_data_s), dev, chunk=1 << 16)
+    th = workloads.random_start(cfg, 0).numpy()
+    v = workloads.direction(cfg, 0).numpy()
+    threads = oracle.max_threads()
+    for _ in range(args.warmup):
+        _oracle_sample_time(w, n_mc_s, n_data_s, th, v, threads)
+    times = [_oracle_sample_time(w, n_mc_s, n_data_s, th, v, threads)[0] for _ in range(args.steps)]
+    total = sum(times)
+    ev = (n_mc_s + n_data_s) * args.steps / total
+    sample = f"first {n_mc_s} MC + {n_data_s} data events of the config-{args.config} recipe per step"
+    line = {"impl": "reference", "metric": METRIC, "value": ev, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"config {args.config} ({cfg.name}): R={cfg.n_res} H={cfg.n_hel} C={cfg.n_chan}, "
+                                   f"bounded sample of {n_mc_s}+{n_data_s} events"},
+            "cpu_baseline": {"value": ev, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": ev, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config (1-4, 6); 3 is the target")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--ref-events", type=int, default=5_000_000, help="MC events in the oracle's bounded sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--mc", type=int, default=0, help="override N_mc (experiments only)")
+    ap.add_argument("--data", type=int, default=0, help="override N_data (experiments only)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else max(args.warmup, 1)
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import numpy as np
+    import torch
+    import paper_2403_09225_b200 as pwa
+    import workloads
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU path)")
+    pwa.load()  # raises if libpwa_b200.so is missing
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    base = workloads.CONFIGS[args.config]
+    cfg = base.scaled(args.mc or base.n_mc, args.data or base.n_data)
+    if world > 1:  # every rank holds its own shard: same recipe, rank-specific seed
+        from dataclasses import replace
+        cfg = replace(cfg, index=cfg.index + 1000 * rank)
+    t_gen = time.time()
+    w = workloads.make_workload(cfg, dev)
+    torch.cuda.synchronize()
+    t_gen = time.time() - t_gen
+    m = pwa.Model(w, device=local, borrow=True)
+    P = m.P
+    th_np = workloads.random_start(base, 0).numpy()
+    v_np = workloads.direction(base, 0).numpy()
+    theta = torch.tensor(th_np, device=dev)
+    v = torch.tensor(v_np, device=dev)
+    raw = torch.zeros(4 + 4 * P, dtype=torch.float64, device=dev)
+    events_per_step = cfg.n_mc + cfg.n_data
+    bytes_per_step = pwa.pwa_bytes_per_eval(m.h)
+
+    def step():
+        if world == 1:
+            pwa.pwa_nll_grad_hvp(m.h, theta, v, m.nll_t, m.grad_t, m.hv_t)
+        else:
+            pwa.pwa_raw_sums(m.h, theta, v, raw)
+            dist.all_reduce(raw)
+            pwa.pwa_combine(m.h, raw, v, m.nll_t, m.grad_t, m.hv_t)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.3)
+    pwa.pwa_profile_enable(m.h, True)
+    pwa.pwa_profile_read(m.h)
+    l0 = pwa.pwa_kernel_launches(m.h)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    tw0 = time.time()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    tw1 = time.time()
+    ms = e0.elapsed_time(e1)
+    sweep_ms, sweep_n = pwa.pwa_profile_read(m.h)
+    pwa.pwa_profile_enable(m.h, False)
+    launches = pwa.pwa_kernel_launches(m.h) - l0
+    clocks = sampler.stop(tw0, tw1) if rank == 0 else None
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    nll_dev = m.nll_t.item()
+
+    # ---- end to end through the host-buffer entry point: H2D of theta, v and D2H of nll, grad, hv every step ----
+    th_h, v_h = np.ascontiguousarray(th_np), np.ascontiguousarray(v_np)
+    o_nll, o_g, o_h = np.zeros(1), np.zeros(P), np.zeros(P)
+    for _ in range(2):
+        pwa.pwa_nll_grad_hvp_host(m.h, th_h, v_h, o_nll, o_g, o_h)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        pwa.pwa_nll_grad_hvp_host(m.h, th_h, v_h, o_nll, o_g, o_h)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    peak, peak_src = _peaks()
+    sweep_avg_s = (sweep_ms / max(sweep_n, 1)) * 1e-3
+    achieved = bytes_per_step / sweep_avg_s / 1e9 if sweep_n else None
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")  # ncu dram bytes per sweep launch, written from a capture
+    if os.path.exists(tpath):
+        try:
+            with open(tpath) as f:
+                tj = json.load(f)
+            key = f"config{args.config}:{pwa.pwa_kernel_variant(m.h)}"
+            traffic = tj.get(key)
+        except Exception:
+            traffic = None
+    line = {
+        "metric": METRIC, "value": world * events_per_step * args.steps / (ms * 1e-3), "unit": UNIT,
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"config {args.config} ({cfg.name}): R={cfg.n_res} H={cfg.n_hel} C={cfg.n_chan} "
+                               f"P={cfg.n_par}, N_mc={cfg.n_mc} N_data={cfg.n_data} per GPU"
+                               f"{', weighted data' if cfg.weighted else ''}",
+                   "l2": f"inputs ({bytes_per_step / 1e6:.0f} MB per step) exceed the 126 MB L2; no flush needed"
+                         if bytes_per_step > 2 * 126e6 else "inputs fit in L2 (cache-resident case)",
+                   "kernel_variant": pwa.pwa_kernel_variant(m.h), "parallelism": f"event shards x{world}",
+                   "workload_gen_s": round(t_gen, 1)},
+        "evals_per_s": args.steps / (ms * 1e-3),
+        "nll": nll_dev,
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": (achieved / peak) if achieved else None, "traffic": traffic,
+                     "peak_source": peak_src, "kernel": "sweep", "bytes_per_launch": bytes_per_step,
+                     "avg_launch_ms": sweep_avg_s * 1e3, "launches_timed": sweep_n},
+        "e2e": {"value": world * events_per_step * args.steps / e2e_s, "unit": UNIT,
+                "h2d_bytes_per_step": 2 * P * 8, "d2h_bytes_per_step": (1 + 2 * P) * 8,
+                "ms_per_step": 1e3 * e2e_s / args.steps},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+    }
+    if not args.no_cpu_baseline:
+        import oracle
+        oracle.build()
+        threads = oracle.max_threads()
+        n_mc_s = min(cfg.n_mc, args.ref_events)
+        n_data_s = max(1, n_mc_s * cfg.n_data // cfg.n_mc)
+        dt, out = _oracle_sample_time(w, n_mc_s, n_data_s, th_np, v_np, threads)
+        line["cpu_baseline"] = {"value": (n_mc_s + n_data_s) / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
+                                "sample": f"first {n_mc_s} MC + {n_data_s} data events of the same arrays, one "
+                                          f"NLL+grad+HVP evaluation ({dt:.1f} s)"}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
