@@ -1,6 +1,7 @@
 // pwa_api.cu - the C ABI of include/pwa.h: handle, event store, evaluation entry points.
 #include <cstdio>
 #include <cstring>
+#include <algorithm>
 #include <mutex>
 #include <new>
 
@@ -69,38 +70,52 @@ static size_t generic_smem(int block, int nb) { return (size_t)(block / 32) * ((
 static pwa_status raw_sums_impl(pwa_handle* h, int mode, const double* theta, const double* v, double* raw) {
   const int R = h->n_res;
   if (mode == MODE_FULL && !v) mode = MODE_GRAD;
-  k_prologue<<<(R + 127) / 128, 128, 0, h->stream>>>(theta, mode == MODE_FULL ? v : nullptr, R, h->d_K);
-  h->launches++;
-  if (cudaError_t ce = cudaGetLastError()) return set_error(h, PWA_ERR_CUDA, "launch k_prologue", ce);
-  SweepArgs a;
-  a.s[0] = h->smp[0];
-  a.s[1] = h->smp[1];
-  a.K = h->d_K;
-  a.ch = h->d_ch;
-  a.R = R;
-  a.C = h->n_chan;
-  a.nb = nb_of(R, mode);
-  a.partial = h->d_partial;
-  sweep_fn fn = generic_fn(h->n_hel, mode);
   const bool prof = h->profiling && h->prof_used + 2 <= h->prof_events.size();
-  if (prof) cudaEventRecord(h->prof_events[h->prof_used], h->stream);
-  fn<<<h->grid, h->block, generic_smem(h->block, a.nb), h->stream>>>(a);
-  h->launches++;
-  if (prof) {
-    cudaEventRecord(h->prof_events[h->prof_used + 1], h->stream);
-    h->prof_used += 2;
+  const int packed = h->variant == 1;
+  int nb = 0;
+  if (packed) {
+    // tiled TMA sweep: the per-resonance constants are formed by every block itself (no prologue launch)
+    if (prof) cudaEventRecord(h->prof_events[h->prof_used], h->stream);
+    pwa_status st = tma_launch(h, mode, theta, mode == MODE_FULL ? v : nullptr);
+    if (st != PWA_OK) return st;
+    h->launches++;
+    if (prof) {
+      cudaEventRecord(h->prof_events[h->prof_used + 1], h->stream);
+      h->prof_used += 2;
+    }
+  } else {
+    k_prologue<<<(R + 127) / 128, 128, 0, h->stream>>>(theta, mode == MODE_FULL ? v : nullptr, R, h->d_K);
+    h->launches++;
+    if (cudaError_t ce = cudaGetLastError()) return set_error(h, PWA_ERR_CUDA, "launch k_prologue", ce);
+    SweepArgs a;
+    a.s[0] = h->smp[0];
+    a.s[1] = h->smp[1];
+    a.K = h->d_K;
+    a.ch = h->d_ch;
+    a.R = R;
+    a.C = h->n_chan;
+    a.nb = nb = nb_of(R, mode);
+    a.partial = h->d_partial;
+    sweep_fn fn = generic_fn(h->n_hel, mode);
+    if (prof) cudaEventRecord(h->prof_events[h->prof_used], h->stream);
+    fn<<<h->grid, h->block, generic_smem(h->block, a.nb), h->stream>>>(a);
+    h->launches++;
+    if (prof) {
+      cudaEventRecord(h->prof_events[h->prof_used + 1], h->stream);
+      h->prof_used += 2;
+    }
+    if (cudaError_t ce = cudaGetLastError()) return set_error(h, PWA_ERR_CUDA, "launch sweep kernel", ce);
   }
-  if (cudaError_t ce = cudaGetLastError()) return set_error(h, PWA_ERR_CUDA, "launch sweep kernel", ce);
   const double n_mc = (double)h->smp[0].n;
   switch (mode) {
     case MODE_NLL:
-      k_reduce_unpack<MODE_NLL><<<1, 1024, 0, h->stream>>>(h->d_partial, h->grid, a.nb, R, theta, v, n_mc, h->d_sums, raw);
+      k_reduce_unpack<MODE_NLL><<<1, 1024, 0, h->stream>>>(h->d_partial, h->grid, nb, R, packed, theta, v, n_mc, h->d_sums, raw);
       break;
     case MODE_GRAD:
-      k_reduce_unpack<MODE_GRAD><<<1, 1024, 0, h->stream>>>(h->d_partial, h->grid, a.nb, R, theta, v, n_mc, h->d_sums, raw);
+      k_reduce_unpack<MODE_GRAD><<<1, 1024, 0, h->stream>>>(h->d_partial, h->grid, nb, R, packed, theta, v, n_mc, h->d_sums, raw);
       break;
     default:
-      k_reduce_unpack<MODE_FULL><<<1, 1024, 0, h->stream>>>(h->d_partial, h->grid, a.nb, R, theta, v, n_mc, h->d_sums, raw);
+      k_reduce_unpack<MODE_FULL><<<1, 1024, 0, h->stream>>>(h->d_partial, h->grid, nb, R, packed, theta, v, n_mc, h->d_sums, raw);
       break;
   }
   h->launches++;
@@ -235,29 +250,37 @@ extern "C" pwa_status pwa_create(const pwa_model_desc* m, pwa_handle** out) {
   // ---- launch configuration of the sweep (fixed for the life of the handle) ------------------------
   const int R = h->n_res, P = h->n_par;
   const int nb_full = nb_of(R, MODE_FULL);
-  int block = 256;
-  while (block > 32 && generic_smem(block, nb_full) > 160 * 1024) block /= 2;
-  // the opt-in limit is a property of the function, shared by every handle: always raise it to one fixed cap
-  const size_t smem = 200 * 1024;
-  int occ_min = 1 << 30;
-  for (int mode = 0; mode < 3; ++mode) {
-    sweep_fn fn = generic_fn(h->n_hel, mode);
-    if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess)
-      return fail_create(h, PWA_ERR_CUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(ce));
-    int occ = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, block, generic_smem(block, nb_of(R, mode)));
-    if (occ < 1) occ = 1;
-    if (occ < occ_min) occ_min = occ;
+  if (cudaMalloc(&h->d_ch, sizeof(int) * R) != cudaSuccess) {
+    cudaGetLastError();
+    return fail_create(h, PWA_ERR_OOM, "scratch allocation failed");
   }
-  h->block = block;
-  h->grid = h->num_sms * occ_min;
-  h->variant_name = "generic";
+  why.clear();
+  st = tma_configure(h, why);
+  if (st != PWA_OK) return fail_create(h, st, h->err);
+  if (h->variant == 0) {
+    int block = 256;
+    while (block > 32 && generic_smem(block, nb_full) > 160 * 1024) block /= 2;
+    // the opt-in limit is a property of the function, shared by every handle: always raise it to one fixed cap
+    const size_t smem = 200 * 1024;
+    int occ_min = 1 << 30;
+    for (int mode = 0; mode < 3; ++mode) {
+      sweep_fn fn = generic_fn(h->n_hel, mode);
+      if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess)
+        return fail_create(h, PWA_ERR_CUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(ce));
+      int occ = 0;
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, block, generic_smem(block, nb_of(R, mode)));
+      if (occ < 1) occ = 1;
+      if (occ < occ_min) occ_min = occ;
+    }
+    h->block = block;
+    h->grid = h->num_sms * occ_min;
+    std::snprintf(h->variant_name, sizeof(h->variant_name), "generic(%s)", why.c_str());
+  }
 
-  const size_t pstride = (size_t)nb_full * 32 + 2;
+  const size_t pstride = std::max((size_t)nb_full * 32, (size_t)R * 10) + 2;
   h->partial_doubles = 2 * (size_t)h->grid * pstride;
   const size_t io = 1 + 4 * (size_t)P + 8;
-  bool ok = cudaMalloc(&h->d_ch, sizeof(int) * R) == cudaSuccess &&
-            cudaMalloc(&h->d_K, sizeof(double) * KSTRIDE * R) == cudaSuccess &&
+  bool ok = cudaMalloc(&h->d_K, sizeof(double) * KSTRIDE * R) == cudaSuccess &&
             cudaMalloc(&h->d_partial, sizeof(double) * h->partial_doubles) == cudaSuccess &&
             cudaMalloc(&h->d_sums, sizeof(double) * 2 * pstride) == cudaSuccess &&
             cudaMalloc(&h->d_raw, sizeof(double) * (4 + 4 * (size_t)P)) == cudaSuccess &&

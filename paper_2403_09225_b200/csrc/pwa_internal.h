@@ -7,6 +7,7 @@
 
 #include "../../include/pwa.h"
 #include "pwa_common.cuh"
+#include "pwa_sweep_tma.cuh"
 
 struct pwa_handle {
   int device = 0;
@@ -30,8 +31,12 @@ struct pwa_handle {
 
   // sweep launch configuration (fixed at creation -> deterministic event -> thread map)
   int grid = 0, block = 0;
-  int variant = 0;
-  const char* variant_name = "generic";
+  int variant = 0;  // 0 = generic, 1 = tma (tiled, TMA-staged; pwa_sweep_tma.cuh)
+  char variant_name[64] = "generic";
+  // tma variant: one argument block per mode (they differ in the shared-memory offsets only)
+  pwa::TmaArgs targs[3];
+  size_t tma_smem[3] = {0, 0, 0};
+  int tma_rho = 0;
 
   // device staging for the *_host entry point and the fit driver
   double* d_io = nullptr;   // theta | v | nll | grad | hv   (1 + 4P doubles, padded)
@@ -47,6 +52,12 @@ struct pwa_handle {
 };
 
 namespace pwa {
+// pwa_sweep_tma.cu: kernel lookup, configuration at creation, launch
+typedef void (*tma_fn)(const TmaArgs);
+tma_fn tma_kernel(int H, int rho, int mode);
+int tma_maxw(int rho);
+pwa_status tma_configure(pwa_handle* h, std::string& why);  // sets variant = 1 on success; PWA_OK + why if unsuitable
+pwa_status tma_launch(pwa_handle* h, int mode, const double* theta, const double* v);
 // internal entry points used by the fit driver (enqueue only)
 pwa_status eval(pwa_handle* h, int mode, const double* theta, const double* v, double* nll, double* grad,
                 double* hv);

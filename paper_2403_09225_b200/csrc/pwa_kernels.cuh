@@ -287,13 +287,14 @@ __device__ inline void unpack_res(const Sums5& s, double a, double phi, double M
   h4[3] = 2.0 * t.re;
 }
 
+// packed = 1: partial rows are [R][VPR] + 2 scalars (tiled TMA sweep); packed = 0: [nb][32] + 2 (generic sweep)
 template <int MODE>
 __global__ void __launch_bounds__(1024) k_reduce_unpack(const double* __restrict__ partial, int nblocks, int nb, int R,
-                                                        const double* __restrict__ theta,
+                                                        int packed, const double* __restrict__ theta,
                                                         const double* __restrict__ v, double n_mc,
                                                         double* __restrict__ sums, double* __restrict__ raw) {
   constexpr int VPR = vpr_of(MODE), RPB = rpb_of(MODE);
-  const int nacc = nb * 32, stride = nacc + 2, P = 4 * R;
+  const int nacc = packed ? (MODE == MODE_NLL ? 0 : R * VPR) : nb * 32, stride = nacc + 2, P = 4 * R;
   for (int k = threadIdx.x; k < 2 * stride; k += blockDim.x) {
     const int sample = k / stride, idx = k - sample * stride;
     const double* p = partial + (size_t)sample * nblocks * stride + idx;
@@ -314,9 +315,10 @@ __global__ void __launch_bounds__(1024) k_reduce_unpack(const double* __restrict
   }
   for (int r = threadIdx.x; r < R; r += blockDim.x) {
     const int b = r / RPB, j = r - b * RPB;
+    const int qoff = packed ? r * VPR : b * 32 + j * VPR;
     const double a = theta[4 * r], phi = theta[4 * r + 1], M = theta[4 * r + 2], G = theta[4 * r + 3];
     for (int sample = 0; sample < 2; ++sample) {
-      const double* q = sums + (size_t)sample * stride + b * 32 + j * VPR;
+      const double* q = sums + (size_t)sample * stride + qoff;
       Sums5 s;
       s.P1 = {q[0], q[1]};
       s.P2 = {q[2], q[3]};
