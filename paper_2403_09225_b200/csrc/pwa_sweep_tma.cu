@@ -11,15 +11,15 @@ int tma_maxw(int rho) {
   switch (rho) {
     case 1: return 16;
     case 2: return 16;
-    case 3: return 10;
-    case 4: return 8;
+    case 3: return 12;
+    case 4: return 12;
   }
   return 0;
 }
 
 template <int H, int RHO>
 static tma_fn tma_for_mode(int mode) {
-  constexpr int MAXW = RHO <= 2 ? 16 : (RHO == 3 ? 10 : 8);
+  constexpr int MAXW = RHO <= 2 ? 16 : 12;  // compute warps + the producer warp
   switch (mode) {
     case MODE_NLL: return k_sweep_tma<H, RHO, MODE_NLL, MAXW>;
     case MODE_GRAD: return k_sweep_tma<H, RHO, MODE_GRAD, MAXW>;
@@ -110,7 +110,7 @@ pwa_status tma_configure(pwa_handle* h, std::string& why) {
   }
   if (rho < 1 || rho > 4) { why = "bad PWA_RHO"; return PWA_OK; }
   const int S = (R + rho - 1) / rho;
-  if (S > tma_maxw(rho)) { why = "too many resonances for the tiled kernel"; return PWA_OK; }
+  if (S + 1 > tma_maxw(rho)) { why = "too many resonances for the tiled kernel"; return PWA_OK; }
 
   const int RH = R * H;
   const int nbox = (RH + 255) / 256, rows_box = (RH + nbox - 1) / nbox;
@@ -121,9 +121,9 @@ pwa_status tma_configure(pwa_handle* h, std::string& why) {
     unsigned o = 0;
     off[0] = o; o += 2u * S * NQ * TILE * 16;   // part
     off[1] = o; o += 2u * NQ * TILE * 16;       // tot
-    off[2] = o; o += (unsigned)R * KSTRIDE * 8;  // K
-    off[3] = o; o += up((unsigned)R * 4, 8);     // ch
-    off[4] = o; o += 8u * 16;                    // mbarriers (<= 16 stages)
+    off[2] = o; o += (unsigned)R * KS * 8;       // K
+    off[3] = o;
+    off[4] = o; o += 8u * (2 * 8 + 4);           // mbarriers: full, empty (<= 8 stages each), pf[2], tf[2]
     return up(o, 128);
   };
   unsigned off_full[5];
@@ -133,7 +133,7 @@ pwa_status tma_configure(pwa_handle* h, std::string& why) {
   int sm_smem = 0;
   cudaDeviceGetAttribute(&sm_smem, cudaDevAttrMaxSharedMemoryPerMultiprocessor, h->device);
   int bps = env_int("PWA_BPS", 0);
-  if (bps <= 0) bps = std::max(1, std::min(8, 20 / S));
+  if (bps <= 0) bps = std::max(1, std::min(8, 20 / (S + 1)));
   int stages = 0;
   for (; bps >= 1; --bps) {
     const long long budget = std::min<long long>(dev_smem, sm_smem / bps - 1024);
@@ -154,7 +154,7 @@ pwa_status tma_configure(pwa_handle* h, std::string& why) {
     cudaError_t ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, dev_smem);
     if (ce != cudaSuccess) return set_error(h, PWA_ERR_CUDA, "cudaFuncSetAttribute(tma sweep)", ce);
     int occ = 0;
-    ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, S * 32, smem);
+    ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, (S + 1) * 32, smem);
     if (ce != cudaSuccess || occ < 1) {
       cudaGetLastError();
       why = "tiled kernel cannot be resident (registers / shared memory)";
@@ -167,7 +167,7 @@ pwa_status tma_configure(pwa_handle* h, std::string& why) {
     a.weighted = h->smp[1].weight != nullptr;
     a.stage_bytes = stage_bytes; a.amp_bytes = amp_bytes; a.mass_bytes = mass_bytes;
     const unsigned base = (unsigned)stages * stage_bytes;
-    a.off_part = base + off[0]; a.off_tot = base + off[1]; a.off_K = base + off[2]; a.off_ch = base + off[3];
+    a.off_part = base + off[0]; a.off_tot = base + off[1]; a.off_K = base + off[2];
     a.off_bar = base + off[4];
     a.ch = h->d_ch;
     for (int sidx = 0; sidx < 2; ++sidx) {
@@ -185,7 +185,7 @@ pwa_status tma_configure(pwa_handle* h, std::string& why) {
   const int use_bps = bps_env > 0 ? std::min(bps_env, occ_min) : std::min(bps, occ_min);
   h->variant = 1;
   h->tma_rho = rho;
-  h->block = S * 32;
+  h->block = (S + 1) * 32;
   h->grid = h->num_sms * use_bps;
   std::snprintf(h->variant_name, sizeof(h->variant_name), "tma(rho=%d,S=%d,stages=%d,bps=%d)", rho, S, stages, use_bps);
   return PWA_OK;
