@@ -13,7 +13,7 @@ import sys
 PKG = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libpwa_b200.so")
-SOURCES = ["pwa_api.cu", "pwa_fit.cu", "pwa_sweep_tma.cu"]
+SOURCES = ["pwa_api.cu", "pwa_fit.cu", "pwa_sweep_tma.cu", "pwa_sweep_lanes.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--use_fast_math=false", "-Xcompiler", "-fPIC,-O2", "-shared", "-cudart", "static", "--threads", "0"]
 

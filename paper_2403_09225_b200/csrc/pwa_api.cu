@@ -1,5 +1,6 @@
 // pwa_api.cu - the C ABI of include/pwa.h: handle, event store, evaluation entry points.
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <algorithm>
 #include <mutex>
@@ -71,12 +72,13 @@ static pwa_status raw_sums_impl(pwa_handle* h, int mode, const double* theta, co
   const int R = h->n_res;
   if (mode == MODE_FULL && !v) mode = MODE_GRAD;
   const bool prof = h->profiling && h->prof_used + 2 <= h->prof_events.size();
-  const int packed = h->variant == 1;
+  const int packed = h->variant >= 1;
   int nb = 0;
   if (packed) {
     // tiled TMA sweep: the per-resonance constants are formed by every block itself (no prologue launch)
     if (prof) cudaEventRecord(h->prof_events[h->prof_used], h->stream);
-    pwa_status st = tma_launch(h, mode, theta, mode == MODE_FULL ? v : nullptr);
+    pwa_status st = h->variant == 2 ? lanes_launch(h, mode, theta, mode == MODE_FULL ? v : nullptr)
+                                    : tma_launch(h, mode, theta, mode == MODE_FULL ? v : nullptr);
     if (st != PWA_OK) return st;
     h->launches++;
     if (prof) {
@@ -255,8 +257,21 @@ extern "C" pwa_status pwa_create(const pwa_model_desc* m, pwa_handle** out) {
     return fail_create(h, PWA_ERR_OOM, "scratch allocation failed");
   }
   why.clear();
-  st = tma_configure(h, why);
-  if (st != PWA_OK) return fail_create(h, st, h->err);
+  h->weight_padded = h->owned[5] != nullptr;
+  const char* force = std::getenv("PWA_VARIANT");
+  const bool want_lanes = !force || std::strcmp(force, "lanes") == 0;
+  const bool want_tma = !force || std::strcmp(force, "tma") == 0;
+  if (want_lanes) {
+    st = lanes_configure(h, why);
+    if (st != PWA_OK) return fail_create(h, st, h->err);
+  }
+  if (h->variant == 0 && want_tma) {
+    std::string why2;
+    st = tma_configure(h, why2);
+    if (st != PWA_OK) return fail_create(h, st, h->err);
+    if (h->variant == 0) why = why.empty() ? why2 : why + "; " + why2;
+  }
+  if (h->variant == 0 && force) why = std::string("PWA_VARIANT=") + force + (why.empty() ? "" : "; " + why);
   if (h->variant == 0) {
     int block = 256;
     while (block > 32 && generic_smem(block, nb_full) > 160 * 1024) block /= 2;

@@ -8,6 +8,7 @@
 #include "../../include/pwa.h"
 #include "pwa_common.cuh"
 #include "pwa_sweep_tma.cuh"
+#include "pwa_sweep_lanes.cuh"
 
 struct pwa_handle {
   int device = 0;
@@ -31,12 +32,17 @@ struct pwa_handle {
 
   // sweep launch configuration (fixed at creation -> deterministic event -> thread map)
   int grid = 0, block = 0;
-  int variant = 0;  // 0 = generic, 1 = tma (tiled, TMA-staged; pwa_sweep_tma.cuh)
+  int variant = 0;  // 0 = generic, 1 = tma (pwa_sweep_tma.cuh), 2 = lanes (pwa_sweep_lanes.cuh)
   char variant_name[64] = "generic";
   // tma variant: one argument block per mode (they differ in the shared-memory offsets only)
   pwa::TmaArgs targs[3];
   size_t tma_smem[3] = {0, 0, 0};
   int tma_rho = 0;
+  // lanes variant (pwa_sweep_lanes.cuh)
+  pwa::LaneArgs largs;
+  size_t lanes_smem = 0;
+  int lanes_rho = 0, lanes_log_sw = 0, lanes_nw = 0;
+  bool weight_padded = false;  // the data weights are library-owned and padded to an even length
 
   // device staging for the *_host entry point and the fit driver
   double* d_io = nullptr;   // theta | v | nll | grad | hv   (1 + 4P doubles, padded)
@@ -58,6 +64,14 @@ tma_fn tma_kernel(int H, int rho, int mode);
 int tma_maxw(int rho);
 pwa_status tma_configure(pwa_handle* h, std::string& why);  // sets variant = 1 on success; PWA_OK + why if unsuitable
 pwa_status tma_launch(pwa_handle* h, int mode, const double* theta, const double* v);
+// fp64 matrix [rows][row_stride_bytes / 8], valid extent (cols, rows), box (box_cols, box_rows); out-of-bounds reads give 0
+bool encode_2d(CUtensorMap* m, const void* base, unsigned long long cols, unsigned long long rows,
+               unsigned long long row_stride_bytes, unsigned box_cols, unsigned box_rows, bool swizzle128 = false);
+// pwa_sweep_lanes.cu
+typedef void (*lanes_fn)(const LaneArgs);
+lanes_fn lanes_kernel(int H, int rho, int log_sw, int nw, int mode);
+pwa_status lanes_configure(pwa_handle* h, std::string& why);  // sets variant = 2 on success; PWA_OK + why if unsuitable
+pwa_status lanes_launch(pwa_handle* h, int mode, const double* theta, const double* v);
 // internal entry points used by the fit driver (enqueue only)
 pwa_status eval(pwa_handle* h, int mode, const double* theta, const double* v, double* nll, double* grad,
                 double* hv);

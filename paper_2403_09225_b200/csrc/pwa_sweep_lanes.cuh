@@ -1,0 +1,477 @@
+// pwa_sweep_lanes.cuh - the warp-autonomous sweep kernel of the hot path (SURVEY §8(a) rows a-1 .. a-7), sm_100a.
+//
+// Work decomposition.  A tile is 32 consecutive events.  Tiles reach shared memory through a ring of stages
+// filled by one producer thread with TMA tensor copies (cp.async.bulk.tensor.2d): four boxes of 8 events x all
+// R*H amplitude planes with the 128-byte swizzle (so that the reads below are bank-conflict free), one box for the
+// mass planes, one for the weights; full[stage] / empty[stage] mbarriers track the ring; events beyond the ragged
+// end and the planes of padding resonances are zero-filled by the TMA unit.  Every F element is read from HBM
+// exactly once and is consumed by exactly one thread.
+//
+// A compute warp works on one "pass" at a time: EW = 32 / SW consecutive events of a tile, the R resonances dealt
+// over SW "slices" of RHO resonances each.  lane = s * EW + e (slice s, event e); lane (s, e) owns the resonances
+// r = j * SW + s, j < RHO.  Per pass a lane
+//   forward : B_r = 1/D_r (a-1), G_rh = B_r F_rh, slice-partial A_h = sum c_r G_rh, Adot_h = sum (alpha_r + beta_r B_r) G_rh
+//             (a-2); F is now in registers, the stage is released
+//   exchange: the 2H (4H with the HVP) real partials are summed over the SW slices INSIDE THE WARP by a
+//             reduce-scatter / all-gather over the slice bits of the lane id (shuffles; no shared memory, no
+//             barrier, fixed order)
+//   event   : I = sum |A_h|^2; data: ln I, omega = w / I, kappa = Idot / I  (a-3, a-4)
+//   backward: B S_r = sum_h conj(omega A_h) G_rh, B S'_r = sum_h conj(omega (Adot_h - kappa A_h)) G_rh, and from them the
+//             five compact sums P1, P2, P3, Q1, Q2 of pwa_common.cuh (a-5, a-6) in per-lane registers
+// Warps never wait for one another: the only synchronisation inside the tile loop is the TMA ring.  At the end of
+// each sample the accumulators are summed over the event lanes (butterfly), over the warps of the block (shared
+// memory, fixed order) and written as one partial row per block (a-7, first stage).
+#pragma once
+#include <cuda.h>
+
+#include "pwa_common.cuh"
+
+namespace pwa {
+
+struct alignas(64) LaneArgs {
+  CUtensorMap tm_amp[2], tm_mass[2], tm_wgt[2];  // 0 = MC, 1 = data
+  long long n[2];
+  int weighted;  // data events carry weights
+  const double* theta;
+  const double* v;
+  const int* ch;
+  double* partial;  // [2][gridDim.x][R*NACC + 2]
+  int R, C, stages;
+  int nbox, rows_box;                       // amplitude rows are loaded in nbox boxes of rows_box rows (<= 256)
+  unsigned stage_bytes, sub_bytes, off_mass, off_wgt;  // inside a stage: 4 sub-tiles of sub_bytes, mass, weights
+  unsigned off_K, off_red, off_bar;         // after the stages
+};
+
+namespace lanes {
+
+constexpr int TILE = 32;       // events per tile
+constexpr int SUB = 8;         // events per swizzled sub-tile (128 bytes per amplitude plane)
+constexpr int KS = 10;         // doubles of constants per resonance
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(bar),
+      "r"(parity)
+      : "memory");
+}
+// TMA tensor copy global -> shared, completion counted in bytes on an mbarrier (SASS: UTMALDG)
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(dst),
+      "l"(map), "r"(c0), "r"(c1), "r"(bar)
+      : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
+  asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
+}
+
+// 1/d for normal-range positive d: hardware seed (MUFU.RCP64H) and one cubic Newton step; measured maximum
+// relative error against the IEEE division 2.2e-16 (kernels).  Three DFMA, no slow-path branch.
+__device__ __forceinline__ double fast_rcp(double d) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(d));
+  const double e = fma(-d, y, 1.0);
+  const double p = fma(e, e, e);
+  return fma(y, p, y);
+}
+
+__device__ __forceinline__ double shfl_x(double x, int m) { return __shfl_xor_sync(0xffffffffu, x, m); }
+
+// Sum of v[0..N) over the lanes that differ in the bits MASK, 2 MASK, ..., 16 of the lane id; every lane ends
+// with all N totals.  Even N: one reduce-scatter step (each half of the pair keeps half of the values), recurse,
+// then the matching all-gather step.  Odd N: plain butterfly step.  The order of additions is fixed.
+template <int N, int MASK>
+__device__ __forceinline__ void slice_allreduce(double (&v)[N], int lane) {
+  if constexpr (MASK <= 16) {
+    if constexpr (N % 2 == 0) {
+      constexpr int HF = N / 2;
+      const bool up = (lane & MASK) != 0;
+      double keep[HF];
+#pragma unroll
+      for (int i = 0; i < HF; ++i) {
+        const double send = up ? v[i] : v[i + HF];
+        const double mine = up ? v[i + HF] : v[i];
+        keep[i] = mine + shfl_x(send, MASK);
+      }
+      slice_allreduce<HF, MASK * 2>(keep, lane);
+#pragma unroll
+      for (int i = 0; i < HF; ++i) {
+        const double other = shfl_x(keep[i], MASK);
+        v[i] = up ? other : keep[i];
+        v[i + HF] = up ? keep[i] : other;
+      }
+    } else {
+#pragma unroll
+      for (int i = 0; i < N; ++i) v[i] += shfl_x(v[i], MASK);
+      slice_allreduce<N, MASK * 2>(v, lane);
+    }
+  }
+}
+
+// per-resonance constants, packed in pairs for 128-bit shared loads:
+//   k[0..1] = M^2, (M Gamma)^2   k[2] = M Gamma   k[3] = bits: byte offset of the resonance's mass row in a stage
+//   k[4..5] = c   k[6..7] = alpha   k[8..9] = beta          (definitions: pwa_common.cuh)
+__device__ __forceinline__ void resonance_constants(const double* __restrict__ theta, const double* __restrict__ v,
+                                                    int r, long long mass_off, double* k) {
+  const double a = theta[4 * r], phi = theta[4 * r + 1], M = theta[4 * r + 2], G = theta[4 * r + 3];
+  double s, c;
+  sincos(phi, &s, &c);
+  const cplx e = {c, s};
+  const cplx cc = {a * c, a * s};
+  k[0] = M * M;
+  k[1] = (M * G) * (M * G);
+  k[2] = M * G;
+  k[3] = __longlong_as_double(mass_off);
+  k[4] = cc.re;
+  k[5] = cc.im;
+  cplx al = {0.0, 0.0}, be = {0.0, 0.0};
+  if (v) {
+    const double va = v[4 * r], vp = v[4 * r + 1], vM = v[4 * r + 2], vG = v[4 * r + 3];
+    al = cadd(cscale(e, va), cscale(cmuli(cc), vp));
+    const cplx lam = {-2.0 * M * vM, G * vM + M * vG};
+    be = cmul(cc, lam);
+  }
+  k[6] = al.re;
+  k[7] = al.im;
+  k[8] = be.re;
+  k[9] = be.im;
+}
+
+template <int MODE>
+__host__ __device__ constexpr int nacc_of() {
+  return MODE == MODE_FULL ? 10 : (MODE == MODE_GRAD ? 4 : 0);
+}
+// NW compute warps + 1 producer warp per block; (NW + 1) / 4 warps share one SM sub-partition's 16 K registers,
+// so NW = 7 / 11 / 15 allows 255 / 168 / 128 registers per thread.
+
+// ------------------------------------------------------------------------------------------------------
+template <int H, int RHO, int LOG_SW, int NW, int MODE>
+__global__ void __launch_bounds__((NW + 1) * 32, 1) k_sweep_lanes(const __grid_constant__ LaneArgs a) {
+  constexpr int SW = 1 << LOG_SW;          // slices per warp
+  constexpr int EW = 32 / SW;              // events per pass
+  constexpr int NP = SW;                   // passes per tile
+  constexpr int NV = (MODE == MODE_FULL ? 4 : 2) * H;  // reals exchanged per event and slice
+  constexpr int NACC = nacc_of<MODE>();
+  constexpr int NA = NACC > 0 ? NACC : 1;
+  constexpr int RP = RHO * SW;             // resonances incl. padding
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int R = a.R, stages = a.stages;
+  double* Ks = reinterpret_cast<double*>(smem_raw + a.off_K);    // [RP][KS]
+  double* red = reinterpret_cast<double*>(smem_raw + a.off_red);  // [NW][R*NACC + 2]
+  const uint32_t full0 = smem_u32(smem_raw + a.off_bar), empty0 = full0 + 8 * stages;
+
+  // ---- block setup: constants from theta (and v), barriers -----------------------------------------------
+  for (int r = threadIdx.x; r < RP; r += blockDim.x) {
+    double* k = Ks + r * KS;
+    if (r < R) {
+      resonance_constants(a.theta, MODE == MODE_FULL ? a.v : nullptr, r, (long long)a.off_mass + (long long)a.ch[r] * (TILE * 8), k);
+    } else {  // padding resonance: couples to nothing, propagator finite
+      k[0] = 0.0; k[1] = 1.0; k[2] = 0.0; k[3] = __longlong_as_double((long long)a.off_mass);
+      k[4] = k[5] = k[6] = k[7] = k[8] = k[9] = 0.0;
+    }
+  }
+  if (threadIdx.x == 0) {
+    for (int k = 0; k < stages; ++k) {
+      mbar_init(full0 + 8 * k, 1);
+      mbar_init(empty0 + 8 * k, NP);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  // ---- this block's tile list: MC tiles b, b+G, ... then data tiles b, b+G, ... ------------------------
+  const long long nM = a.n[0], nD = a.n[1];
+  const int tilesM = (int)((nM + TILE - 1) / TILE), tilesD = (int)((nD + TILE - 1) / TILE);
+  const int G = gridDim.x, b = blockIdx.x;
+  const int TmB = b < tilesM ? (tilesM - b + G - 1) / G : 0;
+  const int TdB = b < tilesD ? (tilesD - b + G - 1) / G : 0;
+  const int T = TmB + TdB;
+
+  // ======================================= producer warp ===================================================
+  if (w == NW) {
+    if (lane == 0) {
+      tma_prefetch_desc(&a.tm_amp[0]);
+      tma_prefetch_desc(&a.tm_mass[0]);
+      tma_prefetch_desc(&a.tm_amp[1]);
+      tma_prefetch_desc(&a.tm_mass[1]);
+      const uint32_t tx = 4u * a.sub_bytes + (unsigned)a.C * (TILE * 8);
+      int st = 0, round = 0;
+      for (int k = 0; k < T; ++k) {
+        if (round > 0) mbar_wait(empty0 + 8 * st, (uint32_t)((round - 1) & 1));
+        const int smp = k >= TmB ? 1 : 0;
+        const int i0 = (b + (k - (smp ? TmB : 0)) * G) * TILE;
+        const bool wg = smp == 1 && a.weighted;
+        const uint32_t bar = full0 + 8 * st, dst = smem_u32(smem_raw) + st * a.stage_bytes;
+        mbar_expect_tx(bar, tx + (wg ? TILE * 8u : 0u));
+        for (int q = 0; q < TILE / SUB; ++q)
+          for (int x = 0; x < a.nbox; ++x)
+            tma_load_2d(dst + q * a.sub_bytes + x * a.rows_box * (SUB * 16), &a.tm_amp[smp], 2 * (i0 + q * SUB), x * a.rows_box, bar);
+        tma_load_2d(dst + a.off_mass, &a.tm_mass[smp], i0, 0, bar);
+        if (wg) tma_load_2d(dst + a.off_wgt, &a.tm_wgt[smp], i0, 0, bar);
+        if (++st == stages) {
+          st = 0;
+          ++round;
+        }
+      }
+    }
+    return;
+  }
+
+  // ======================================= compute warps ===================================================
+  const int s = lane >> (5 - LOG_SW), e = lane & (EW - 1);
+  double acc[RHO][NA];
+  double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+  for (int j = 0; j < RHO; ++j)
+#pragma unroll
+    for (int q = 0; q < NA; ++q) acc[j][q] = 0.0;
+  // Byte offset of (resonance j, helicity h, this lane's event) inside a sub-tile for the first EW-event column of
+  // the sub-tile: plane row * 128 + ((e ^ (row & 7)) << 4)  (128-byte swizzle: the 16-byte chunk index is XORed with
+  // the row index modulo 8).  The column's chunk base cb (a multiple of EW) enters as one more XOR: (cb + e) ^ x
+  // = cb ^ (e ^ x).
+  static_assert(EW <= SUB, "a pass must not span sub-tiles");
+  unsigned foff[RHO][H];
+#pragma unroll
+  for (int j = 0; j < RHO; ++j)
+#pragma unroll
+    for (int h = 0; h < H; ++h) {
+      const unsigned row = (unsigned)((j * SW + s) * H + h);
+      foff[j][h] = row * (SUB * 16) + (((unsigned)e ^ (row & 7u)) << 4);
+    }
+  const double* lane_k = Ks + s * KS;
+
+  // pass g = w + k NW  ->  local tile t = g / NP, column col = g % NP
+  int t = w / NP, col = w % NP;
+  int st = t % stages, ph = (t / stages) & 1;
+
+  for (int smp = 0; smp < 2; ++smp) {
+    const int t_end = smp ? T : TmB;
+    const long long n = smp ? nD : nM;
+    const bool weighted = smp == 1 && a.weighted;
+#pragma unroll 1
+    while (t < t_end) {
+      const long long i0 = (long long)(b + (t - (smp ? TmB : 0)) * G) * TILE;
+      const int ev = col * EW + e;
+      const bool valid = i0 + ev < n;
+      mbar_wait(full0 + 8 * st, (uint32_t)ph);
+      const unsigned char* sp = smem_raw + (size_t)st * a.stage_bytes;
+      // sub-tile of this column and the XOR term of its chunk base
+      const unsigned char* fp = sp + (unsigned)((col * EW) / SUB) * a.sub_bytes;
+      const unsigned cbx = (unsigned)((col * EW) % SUB) << 4;
+      double wt = 1.0;
+      if (weighted) wt = reinterpret_cast<const double*>(sp + a.off_wgt)[ev];
+
+      // ---------------- forward ----------------
+      double2 Gr[RHO][H], Br[RHO];
+      double x[NV];  // slice partials: A_h (re, im) [then Adot_h (re, im)]
+#pragma unroll
+      for (int j = 0; j < RHO; ++j) {
+        const double2* kk = reinterpret_cast<const double2*>(lane_k + j * (SW * KS));
+        const double2 k01 = kk[0], k23 = kk[1], c = kk[2];
+        const double m = *reinterpret_cast<const double*>(sp + (unsigned)__double_as_longlong(k23.y) + ev * 8);
+        const double xx = fma(-m, m, k01.x);
+        double den = fma(xx, xx, k01.y);
+        den = valid ? den : 1.0;  // lanes beyond the ragged end stay finite
+        const double u = fast_rcp(den);
+        const double br = xx * u, bi = k23.x * u;  // B = conj(D)/|D|^2
+        Br[j] = make_double2(br, bi);
+        if (MODE == MODE_NLL) {
+          const double zr = fma(c.x, br, -(c.y * bi)), zi = fma(c.x, bi, c.y * br);
+#pragma unroll
+          for (int h = 0; h < H; ++h) {
+            const double2 F = *reinterpret_cast<const double2*>(fp + (foff[j][h] ^ cbx));
+            if (j == 0) {
+              x[2 * h] = fma(zr, F.x, -(zi * F.y));
+              x[2 * h + 1] = fma(zr, F.y, zi * F.x);
+            } else {
+              x[2 * h] = fma(zr, F.x, fma(-zi, F.y, x[2 * h]));
+              x[2 * h + 1] = fma(zr, F.y, fma(zi, F.x, x[2 * h + 1]));
+            }
+          }
+        } else {
+          double wr = 0.0, wi = 0.0;
+          if (MODE == MODE_FULL) {  // zdot = (alpha + beta B) B
+            const double2 al = kk[3], be = kk[4];
+            wr = fma(be.x, br, fma(-be.y, bi, al.x));
+            wi = fma(be.x, bi, fma(be.y, br, al.y));
+          }
+#pragma unroll
+          for (int h = 0; h < H; ++h) {
+            const double2 F = *reinterpret_cast<const double2*>(fp + (foff[j][h] ^ cbx));
+            const double gx = fma(br, F.x, -(bi * F.y)), gy = fma(br, F.y, bi * F.x);
+            Gr[j][h] = make_double2(gx, gy);
+            if (j == 0) {
+              x[2 * h] = fma(c.x, gx, -(c.y * gy));
+              x[2 * h + 1] = fma(c.x, gy, c.y * gx);
+              if (MODE == MODE_FULL) {
+                x[2 * H + 2 * h] = fma(wr, gx, -(wi * gy));
+                x[2 * H + 2 * h + 1] = fma(wr, gy, wi * gx);
+              }
+            } else {
+              x[2 * h] = fma(c.x, gx, fma(-c.y, gy, x[2 * h]));
+              x[2 * h + 1] = fma(c.x, gy, fma(c.y, gx, x[2 * h + 1]));
+              if (MODE == MODE_FULL) {
+                x[2 * H + 2 * h] = fma(wr, gx, fma(-wi, gy, x[2 * H + 2 * h]));
+                x[2 * H + 2 * h + 1] = fma(wr, gy, fma(wi, gx, x[2 * H + 2 * h + 1]));
+              }
+            }
+          }
+        }
+      }
+      // everything this pass needs from the stage is in registers: hand the column back to the producer
+      __syncwarp();
+      if (lane == 0) mbar_arrive(empty0 + 8 * st);
+
+      // ---------------- exchange over the slices ----------------
+      slice_allreduce<NV, EW>(x, lane);
+
+      // ---------------- event: I, and for data ln I, omega, kappa ----------------
+      double I = 0.0;
+#pragma unroll
+      for (int h = 0; h < H; ++h)
+        I = h == 0 ? fma(x[0], x[0], x[1] * x[1]) : fma(x[2 * h], x[2 * h], fma(x[2 * h + 1], x[2 * h + 1], I));
+      if (smp == 0) {
+        s0 += I;  // lanes beyond the ragged end read zero-filled F: I = 0 and no contribution below
+      } else {
+        const double wv = valid ? wt : 0.0;
+        const double Iv = valid ? I : 1.0;
+        const double inv = 1.0 / Iv;
+        const double om = wv * inv;
+        s0 = fma(wv, log(Iv), s0);
+        s1 += wv;
+        double kap = 0.0;
+        if (MODE == MODE_FULL) {
+          double Idot = 0.0;
+#pragma unroll
+          for (int h = 0; h < H; ++h)
+            Idot = fma(x[2 * h], x[2 * H + 2 * h], fma(x[2 * h + 1], x[2 * H + 2 * h + 1], Idot));
+          kap = 2.0 * Idot * inv;
+        }
+#pragma unroll
+        for (int h = 0; h < H; ++h) {
+          if (MODE == MODE_FULL) {
+            x[2 * H + 2 * h] = om * fma(-kap, x[2 * h], x[2 * H + 2 * h]);
+            x[2 * H + 2 * h + 1] = om * fma(-kap, x[2 * h + 1], x[2 * H + 2 * h + 1]);
+          }
+          x[2 * h] *= om;
+          x[2 * h + 1] *= om;
+        }
+      }
+
+      // ---------------- backward ----------------
+      if (MODE != MODE_NLL) {
+#pragma unroll
+        for (int j = 0; j < RHO; ++j) {
+          const double br = Br[j].x, bi = Br[j].y;
+          // t1 = B S = sum_h conj(A_h) G_h ;  u1 = B S' = sum_h conj(D_h) G_h
+          double t1r, t1i, u1r = 0.0, u1i = 0.0;
+          {
+            const double2 g = Gr[j][0];
+            t1r = fma(x[0], g.x, x[1] * g.y);
+            t1i = fma(x[0], g.y, -(x[1] * g.x));
+            if (MODE == MODE_FULL) {
+              u1r = fma(x[2 * H], g.x, x[2 * H + 1] * g.y);
+              u1i = fma(x[2 * H], g.y, -(x[2 * H + 1] * g.x));
+            }
+          }
+#pragma unroll
+          for (int h = 1; h < H; ++h) {
+            const double2 g = Gr[j][h];
+            t1r = fma(x[2 * h], g.x, fma(x[2 * h + 1], g.y, t1r));
+            t1i = fma(x[2 * h], g.y, fma(-x[2 * h + 1], g.x, t1i));
+            if (MODE == MODE_FULL) {
+              u1r = fma(x[2 * H + 2 * h], g.x, fma(x[2 * H + 2 * h + 1], g.y, u1r));
+              u1i = fma(x[2 * H + 2 * h], g.y, fma(-x[2 * H + 2 * h + 1], g.x, u1i));
+            }
+          }
+          acc[j][0] += t1r;  // P1
+          acc[j][1] += t1i;
+          if (MODE == MODE_GRAD) {
+            acc[j][2] = fma(br, t1r, fma(-bi, t1i, acc[j][2]));  // P2
+            acc[j][3] = fma(br, t1i, fma(bi, t1r, acc[j][3]));
+          } else {
+            const double t2r = fma(br, t1r, -(bi * t1i)), t2i = fma(br, t1i, bi * t1r);
+            acc[j][2] += t2r;  // P2
+            acc[j][3] += t2i;
+            acc[j][4] = fma(br, t2r, fma(-bi, t2i, acc[j][4]));  // P3
+            acc[j][5] = fma(br, t2i, fma(bi, t2r, acc[j][5]));
+            acc[j][6] += u1r;  // Q1
+            acc[j][7] += u1i;
+            acc[j][8] = fma(br, u1r, fma(-bi, u1i, acc[j][8]));  // Q2
+            acc[j][9] = fma(br, u1i, fma(bi, u1r, acc[j][9]));
+          }
+        }
+      }
+
+      // ---------------- next pass of this warp ----------------
+      col += NW;
+      while (col >= NP) {
+        col -= NP;
+        ++t;
+        if (++st == stages) {
+          st = 0;
+          ph ^= 1;
+        }
+      }
+    }
+
+    // ---- end of a sample: fixed-order butterfly over the event lanes, fixed-order sum over the warps, one
+    //      partial row per block --------------------------------------------------------------------------------
+    const int row_len = R * NACC + 2;
+    double* mine = red + (size_t)w * row_len;
+#pragma unroll
+    for (int j = 0; j < RHO; ++j) {
+      const int r = j * SW + s;
+#pragma unroll
+      for (int q = 0; q < NACC; ++q) {
+        double tsum = acc[j][q];
+#pragma unroll
+        for (int m = 1; m < EW; m <<= 1) tsum += shfl_x(tsum, m);
+        if (e == 0 && r < R) mine[r * NACC + q] = tsum;
+        acc[j][q] = 0.0;
+      }
+    }
+    {
+      double t0 = s0, t1 = s1;
+#pragma unroll
+      for (int m = 1; m < EW; m <<= 1) {
+        t0 += shfl_x(t0, m);
+        t1 += shfl_x(t1, m);
+      }
+      if (lane == 0) {  // slice 0, event lane 0
+        mine[R * NACC] = t0;
+        mine[R * NACC + 1] = t1;
+      }
+      s0 = s1 = 0.0;
+    }
+    asm volatile("bar.sync 1, %0;" ::"n"(NW * 32) : "memory");
+    double* out = a.partial + ((size_t)smp * gridDim.x + blockIdx.x) * (size_t)row_len;
+    for (int k = threadIdx.x; k < row_len; k += NW * 32) {
+      double tsum = red[k];
+      for (int ww = 1; ww < NW; ++ww) tsum += red[(size_t)ww * row_len + k];
+      out[k] = tsum;
+    }
+    asm volatile("bar.sync 1, %0;" ::"n"(NW * 32) : "memory");
+  }
+}
+
+}  // namespace lanes
+}  // namespace pwa

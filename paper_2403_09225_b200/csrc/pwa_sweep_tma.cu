@@ -66,8 +66,8 @@ static encode_fn get_encode() {
 }
 
 // fp64 matrix [rows][row_stride_bytes / 8], valid extent (cols, rows), box (box_cols, box_rows); OOB reads give 0
-static bool encode_2d(CUtensorMap* m, const void* base, unsigned long long cols, unsigned long long rows,
-                      unsigned long long row_stride_bytes, unsigned box_cols, unsigned box_rows) {
+bool encode_2d(CUtensorMap* m, const void* base, unsigned long long cols, unsigned long long rows,
+               unsigned long long row_stride_bytes, unsigned box_cols, unsigned box_rows, bool swizzle128) {
   encode_fn fn = get_encode();
   if (!fn) return false;
   cuuint64_t dims[2] = {cols, rows};
@@ -75,7 +75,8 @@ static bool encode_2d(CUtensorMap* m, const void* base, unsigned long long cols,
   cuuint32_t box[2] = {box_cols, box_rows};
   cuuint32_t es[2] = {1, 1};
   return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void*>(base), dims, strides, box, es,
-            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+            CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
