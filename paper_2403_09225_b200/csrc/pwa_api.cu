@@ -75,10 +75,9 @@ static pwa_status raw_sums_impl(pwa_handle* h, int mode, const double* theta, co
   const int packed = h->variant >= 1;
   int nb = 0;
   if (packed) {
-    // tiled TMA sweep: the per-resonance constants are formed by every block itself (no prologue launch)
+    // lanes sweep: the per-resonance constants are formed by every block itself (no prologue launch)
     if (prof) cudaEventRecord(h->prof_events[h->prof_used], h->stream);
-    pwa_status st = h->variant == 2 ? lanes_launch(h, mode, theta, mode == MODE_FULL ? v : nullptr)
-                                    : tma_launch(h, mode, theta, mode == MODE_FULL ? v : nullptr);
+    pwa_status st = lanes_launch(h, mode, theta, mode == MODE_FULL ? v : nullptr);
     if (st != PWA_OK) return st;
     h->launches++;
     if (prof) {
@@ -260,16 +259,9 @@ extern "C" pwa_status pwa_create(const pwa_model_desc* m, pwa_handle** out) {
   h->weight_padded = h->owned[5] != nullptr;
   const char* force = std::getenv("PWA_VARIANT");
   const bool want_lanes = !force || std::strcmp(force, "lanes") == 0;
-  const bool want_tma = !force || std::strcmp(force, "tma") == 0;
   if (want_lanes) {
     st = lanes_configure(h, why);
     if (st != PWA_OK) return fail_create(h, st, h->err);
-  }
-  if (h->variant == 0 && want_tma) {
-    std::string why2;
-    st = tma_configure(h, why2);
-    if (st != PWA_OK) return fail_create(h, st, h->err);
-    if (h->variant == 0) why = why.empty() ? why2 : why + "; " + why2;
   }
   if (h->variant == 0 && force) why = std::string("PWA_VARIANT=") + force + (why.empty() ? "" : "; " + why);
   if (h->variant == 0) {

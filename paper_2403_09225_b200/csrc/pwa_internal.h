@@ -7,7 +7,6 @@
 
 #include "../../include/pwa.h"
 #include "pwa_common.cuh"
-#include "pwa_sweep_tma.cuh"
 #include "pwa_sweep_lanes.cuh"
 
 struct pwa_handle {
@@ -32,16 +31,12 @@ struct pwa_handle {
 
   // sweep launch configuration (fixed at creation -> deterministic event -> thread map)
   int grid = 0, block = 0;
-  int variant = 0;  // 0 = generic, 1 = tma (pwa_sweep_tma.cuh), 2 = lanes (pwa_sweep_lanes.cuh)
+  int variant = 0;  // 0 = generic (pwa_kernels.cuh), 2 = lanes (pwa_sweep_lanes.cuh)
   char variant_name[64] = "generic";
-  // tma variant: one argument block per mode (they differ in the shared-memory offsets only)
-  pwa::TmaArgs targs[3];
-  size_t tma_smem[3] = {0, 0, 0};
-  int tma_rho = 0;
   // lanes variant (pwa_sweep_lanes.cuh)
   pwa::LaneArgs largs;
   size_t lanes_smem = 0;
-  int lanes_rho = 0, lanes_log_sw = 0, lanes_nw = 0;
+  int lanes_combo = -1;
   bool weight_padded = false;  // the data weights are library-owned and padded to an even length
 
   // device staging for the *_host entry point and the fit driver
@@ -58,18 +53,22 @@ struct pwa_handle {
 };
 
 namespace pwa {
-// pwa_sweep_tma.cu: kernel lookup, configuration at creation, launch
-typedef void (*tma_fn)(const TmaArgs);
-tma_fn tma_kernel(int H, int rho, int mode);
-int tma_maxw(int rho);
-pwa_status tma_configure(pwa_handle* h, std::string& why);  // sets variant = 1 on success; PWA_OK + why if unsuitable
-pwa_status tma_launch(pwa_handle* h, int mode, const double* theta, const double* v);
 // fp64 matrix [rows][row_stride_bytes / 8], valid extent (cols, rows), box (box_cols, box_rows); out-of-bounds reads give 0
 bool encode_2d(CUtensorMap* m, const void* base, unsigned long long cols, unsigned long long rows,
                unsigned long long row_stride_bytes, unsigned box_cols, unsigned box_rows, bool swizzle128 = false);
 // pwa_sweep_lanes.cu
 typedef void (*lanes_fn)(const LaneArgs);
-lanes_fn lanes_kernel(int H, int rho, int log_sw, int nw, int mode);
+struct LanesCombo {
+  int rho, log_sw, nw;  // resonances per lane, log2(slices per warp), compute warps per block
+};
+// instantiated (RHO, LOG_SW, NW) triples (pwa_sweep_lanes_inst.cu); capacity RHO << LOG_SW resonances
+constexpr LanesCombo kLanesCombos[] = {{1, 2, 15}, {2, 3, 15}, {3, 2, 11}, {4, 3, 7}, {4, 4, 7}, {4, 5, 7}};
+constexpr int kNumLanesCombos = sizeof(kLanesCombos) / sizeof(kLanesCombos[0]);
+lanes_fn lanes_kernel_h1(int combo, int mode);
+lanes_fn lanes_kernel_h2(int combo, int mode);
+lanes_fn lanes_kernel_h3(int combo, int mode);
+lanes_fn lanes_kernel_h4(int combo, int mode);
+lanes_fn lanes_kernel(int H, int combo, int mode);
 pwa_status lanes_configure(pwa_handle* h, std::string& why);  // sets variant = 2 on success; PWA_OK + why if unsuitable
 pwa_status lanes_launch(pwa_handle* h, int mode, const double* theta, const double* v);
 // internal entry points used by the fit driver (enqueue only)

@@ -8,28 +8,20 @@
 namespace pwa {
 
 namespace {
-struct Combo {
-  int rho, log_sw, nw;
-};
-// instantiated (RHO, LOG_SW, NW) triples, in order of preference; capacity RHO << LOG_SW resonances
-constexpr Combo kCombos[] = {{4, 3, 7}, {4, 3, 11}, {2, 4, 15}, {2, 4, 11}};
+typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                              const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                              CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-template <int H, int RHO, int LOG_SW, int NW>
-lanes_fn for_mode(int mode) {
-  switch (mode) {
-    case MODE_NLL: return lanes::k_sweep_lanes<H, RHO, LOG_SW, NW, MODE_NLL>;
-    case MODE_GRAD: return lanes::k_sweep_lanes<H, RHO, LOG_SW, NW, MODE_GRAD>;
-    default: return lanes::k_sweep_lanes<H, RHO, LOG_SW, NW, MODE_FULL>;
-  }
-}
-
-template <int H>
-lanes_fn for_combo(int rho, int log_sw, int nw, int mode) {
-  if (rho == 4 && log_sw == 3 && nw == 7) return for_mode<H, 4, 3, 7>(mode);
-  if (rho == 4 && log_sw == 3 && nw == 11) return for_mode<H, 4, 3, 11>(mode);
-  if (rho == 2 && log_sw == 4 && nw == 15) return for_mode<H, 2, 4, 15>(mode);
-  if (rho == 2 && log_sw == 4 && nw == 11) return for_mode<H, 2, 4, 11>(mode);
-  return nullptr;
+encode_fn get_encode() {
+  static encode_fn fn = nullptr;
+  if (fn) return fn;
+  void* p = nullptr;
+  cudaDriverEntryPointQueryResult q;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+      q != cudaDriverEntryPointSuccess)
+    return nullptr;
+  fn = reinterpret_cast<encode_fn>(p);
+  return fn;
 }
 
 int env_int(const char* name, int dflt) {
@@ -39,9 +31,26 @@ int env_int(const char* name, int dflt) {
 inline unsigned up(unsigned x, unsigned m) { return (x + m - 1) / m * m; }
 }  // namespace
 
-lanes_fn lanes_kernel(int H, int rho, int log_sw, int nw, int mode) {
+bool encode_2d(CUtensorMap* m, const void* base, unsigned long long cols, unsigned long long rows,
+               unsigned long long row_stride_bytes, unsigned box_cols, unsigned box_rows, bool swizzle128) {
+  encode_fn fn = get_encode();
+  if (!fn) return false;
+  cuuint64_t dims[2] = {cols, rows};
+  cuuint64_t strides[1] = {row_stride_bytes};
+  cuuint32_t box[2] = {box_cols, box_rows};
+  cuuint32_t es[2] = {1, 1};
+  return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void*>(base), dims, strides, box, es,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+            CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+lanes_fn lanes_kernel(int H, int combo, int mode) {
+  if (combo < 0 || combo >= kNumLanesCombos) return nullptr;
   switch (H) {
-    case 2: return for_combo<2>(rho, log_sw, nw, mode);
+    case 1: return lanes_kernel_h1(combo, mode);
+    case 2: return lanes_kernel_h2(combo, mode);
+    case 3: return lanes_kernel_h3(combo, mode);
+    case 4: return lanes_kernel_h4(combo, mode);
   }
   return nullptr;
 }
@@ -56,28 +65,28 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
       return PWA_OK;
     }
   }
-  int rho = env_int("PWA_RHO", 0), log_sw = env_int("PWA_LOGSW", -1), nw = env_int("PWA_NW", 0);
-  if (rho == 0 || log_sw < 0 || nw == 0) {  // smallest padded capacity; ties go to the earlier table entry
+  // smallest padded capacity among the instantiated combos (ties: the earlier entry); PWA_COMBO forces one
+  int combo = env_int("PWA_COMBO", -1);
+  if (combo < 0) {
     int best = -1;
-    for (const Combo& c : kCombos) {
-      const int cap = c.rho << c.log_sw;
-      if (cap < R || !lanes_kernel(H, c.rho, c.log_sw, c.nw, MODE_FULL)) continue;
-      if (rho && c.rho != rho) continue;
-      if (log_sw >= 0 && c.log_sw != log_sw) continue;
-      if (nw && c.nw != nw) continue;
-      if (best < 0 || cap < best) { best = cap; rho = c.rho; log_sw = c.log_sw; nw = c.nw; }
+    for (int k = 0; k < kNumLanesCombos; ++k) {
+      const int cap = kLanesCombos[k].rho << kLanesCombos[k].log_sw;
+      if (cap >= R && (best < 0 || cap < best)) { best = cap; combo = k; }
     }
-    if (best < 0) { why = "no lanes-kernel instance for this (n_res, n_hel)"; return PWA_OK; }
   }
-  if (!lanes_kernel(H, rho, log_sw, nw, MODE_FULL) || (rho << log_sw) < R) { why = "no lanes-kernel instance"; return PWA_OK; }
+  if (H > 4 || !lanes_kernel(H, combo, MODE_FULL) || (kLanesCombos[combo].rho << kLanesCombos[combo].log_sw) < R) {
+    why = "no lanes-kernel instance for this (n_res, n_hel)";
+    return PWA_OK;
+  }
+  const int rho = kLanesCombos[combo].rho, log_sw = kLanesCombos[combo].log_sw, nw = kLanesCombos[combo].nw;
   const int SW = 1 << log_sw, RP = rho * SW, NW = nw;
 
-  // amplitude rows incl. the zero-filled planes of padding resonances, in nbox boxes of rows_box (<= 256, x8) rows
-  const int rows_need = up((unsigned)RP * H, 8);
-  const int nbox = (rows_need + 255) / 256, rows_box = (int)up((unsigned)((rows_need + nbox - 1) / nbox), 8);
-  const unsigned sub_bytes = (unsigned)nbox * rows_box * lanes::SUB * 16;  // multiple of 1024: swizzle atom alignment
-  const unsigned off_mass = (lanes::TILE / lanes::SUB) * sub_bytes, off_wgt = off_mass + (unsigned)C * lanes::TILE * 8;
-  const unsigned stage_bytes = up(off_wgt + lanes::TILE * 8, 1024);
+  // amplitude rows incl. the zero-filled planes of padding resonances, in nbox boxes of rows_box (<= 256) rows
+  const int rows_need = RP * H;
+  const int nbox = (rows_need + 255) / 256, rows_box = (rows_need + nbox - 1) / nbox;
+  const unsigned amp_bytes = (unsigned)nbox * rows_box * lanes::TILE * 16;
+  const unsigned off_mass = amp_bytes, off_wgt = off_mass + (unsigned)C * lanes::TILE * 8;
+  const unsigned stage_bytes = up(off_wgt + lanes::TILE * 8, 128);
   const unsigned k_bytes = up((unsigned)RP * lanes::KS * 8, 128);
   const unsigned red_bytes = up((unsigned)NW * (R * 10 + 2) * 8, 128);
   const unsigned fixed = k_bytes + red_bytes + 8u * 2 * 8 + 128;
@@ -90,7 +99,7 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
   const size_t smem = (size_t)stages * stage_bytes + fixed;
 
   for (int mode = 0; mode < 3; ++mode) {
-    lanes_fn fn = lanes_kernel(H, rho, log_sw, nw, mode);
+    lanes_fn fn = lanes_kernel(H, combo, mode);
     cudaError_t ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, dev_smem);
     if (ce != cudaSuccess) return set_error(h, PWA_ERR_CUDA, "cudaFuncSetAttribute(lanes sweep)", ce);
     int occ = 0;
@@ -108,7 +117,7 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
     const SampleDev& d = h->smp[sidx];
     a.n[sidx] = d.n;
     bool ok = encode_2d(&a.tm_amp[sidx], d.amp, 2ull * d.n, (unsigned long long)R * H, (unsigned long long)d.stride * 16,
-                        2 * lanes::SUB, rows_box, true) &&
+                        2 * lanes::TILE, rows_box, false) &&
               encode_2d(&a.tm_mass[sidx], d.mass, (unsigned long long)d.n, (unsigned long long)C,
                         (unsigned long long)d.stride * 8, lanes::TILE, C);
     if (ok && d.weight)
@@ -119,12 +128,12 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
   a.ch = h->d_ch;
   a.R = R; a.C = C; a.stages = stages;
   a.nbox = nbox; a.rows_box = rows_box;
-  a.stage_bytes = stage_bytes; a.sub_bytes = sub_bytes; a.off_mass = off_mass; a.off_wgt = off_wgt;
+  a.stage_bytes = stage_bytes; a.amp_bytes = amp_bytes; a.off_mass = off_mass; a.off_wgt = off_wgt;
   a.off_K = (unsigned)stages * stage_bytes;
   a.off_red = a.off_K + k_bytes;
   a.off_bar = a.off_red + red_bytes;
   h->lanes_smem = smem;
-  h->lanes_rho = rho; h->lanes_log_sw = log_sw; h->lanes_nw = nw;
+  h->lanes_combo = combo;
   h->variant = 2;
   h->block = (NW + 1) * 32;
   h->grid = h->num_sms;
@@ -137,7 +146,7 @@ pwa_status lanes_launch(pwa_handle* h, int mode, const double* theta, const doub
   a.theta = theta;
   a.v = v;
   a.partial = h->d_partial;
-  lanes_fn fn = lanes_kernel(h->n_hel, h->lanes_rho, h->lanes_log_sw, h->lanes_nw, mode);
+  lanes_fn fn = lanes_kernel(h->n_hel, h->lanes_combo, mode);
   fn<<<h->grid, h->block, h->lanes_smem, h->stream>>>(a);
   if (cudaError_t ce = cudaGetLastError()) return set_error(h, PWA_ERR_CUDA, "launch lanes sweep kernel", ce);
   return PWA_OK;

@@ -1,11 +1,11 @@
 // pwa_sweep_lanes.cuh - the warp-autonomous sweep kernel of the hot path (SURVEY §8(a) rows a-1 .. a-7), sm_100a.
 //
 // Work decomposition.  A tile is 32 consecutive events.  Tiles reach shared memory through a ring of stages
-// filled by one producer thread with TMA tensor copies (cp.async.bulk.tensor.2d): four boxes of 8 events x all
-// R*H amplitude planes with the 128-byte swizzle (so that the reads below are bank-conflict free), one box for the
-// mass planes, one for the weights; full[stage] / empty[stage] mbarriers track the ring; events beyond the ragged
-// end and the planes of padding resonances are zero-filled by the TMA unit.  Every F element is read from HBM
-// exactly once and is consumed by exactly one thread.
+// filled by one producer thread with TMA tensor copies (cp.async.bulk.tensor.2d): one box of 32 events x all R*H
+// amplitude planes (512 contiguous bytes per plane; narrower boxes were measured to cap the feed at 4.5 TB/s), one
+// box for the mass planes, one for the weights; full[stage] / empty[stage] mbarriers track the ring; events beyond
+// the ragged end and the planes of padding resonances are zero-filled by the TMA unit.  Every F element is read
+// from HBM exactly once and is consumed by exactly one thread.
 //
 // A compute warp works on one "pass" at a time: EW = 32 / SW consecutive events of a tile, the R resonances dealt
 // over SW "slices" of RHO resonances each.  lane = s * EW + e (slice s, event e); lane (s, e) owns the resonances
@@ -38,14 +38,13 @@ struct alignas(64) LaneArgs {
   double* partial;  // [2][gridDim.x][R*NACC + 2]
   int R, C, stages;
   int nbox, rows_box;                       // amplitude rows are loaded in nbox boxes of rows_box rows (<= 256)
-  unsigned stage_bytes, sub_bytes, off_mass, off_wgt;  // inside a stage: 4 sub-tiles of sub_bytes, mass, weights
+  unsigned stage_bytes, amp_bytes, off_mass, off_wgt;  // inside a stage: amplitude planes [rows][32 events], mass, weights
   unsigned off_K, off_red, off_bar;         // after the stages
 };
 
 namespace lanes {
 
 constexpr int TILE = 32;       // events per tile
-constexpr int SUB = 8;         // events per swizzled sub-tile (128 bytes per amplitude plane)
 constexpr int KS = 10;         // doubles of constants per resonance
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -212,7 +211,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_sweep_lanes(const __grid_c
       tma_prefetch_desc(&a.tm_mass[0]);
       tma_prefetch_desc(&a.tm_amp[1]);
       tma_prefetch_desc(&a.tm_mass[1]);
-      const uint32_t tx = 4u * a.sub_bytes + (unsigned)a.C * (TILE * 8);
+      const uint32_t tx = a.amp_bytes + (unsigned)a.C * (TILE * 8);
       int st = 0, round = 0;
       for (int k = 0; k < T; ++k) {
         if (round > 0) mbar_wait(empty0 + 8 * st, (uint32_t)((round - 1) & 1));
@@ -221,9 +220,8 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_sweep_lanes(const __grid_c
         const bool wg = smp == 1 && a.weighted;
         const uint32_t bar = full0 + 8 * st, dst = smem_u32(smem_raw) + st * a.stage_bytes;
         mbar_expect_tx(bar, tx + (wg ? TILE * 8u : 0u));
-        for (int q = 0; q < TILE / SUB; ++q)
-          for (int x = 0; x < a.nbox; ++x)
-            tma_load_2d(dst + q * a.sub_bytes + x * a.rows_box * (SUB * 16), &a.tm_amp[smp], 2 * (i0 + q * SUB), x * a.rows_box, bar);
+        for (int x = 0; x < a.nbox; ++x)
+          tma_load_2d(dst + x * a.rows_box * (TILE * 16), &a.tm_amp[smp], 2 * i0, x * a.rows_box, bar);
         tma_load_2d(dst + a.off_mass, &a.tm_mass[smp], i0, 0, bar);
         if (wg) tma_load_2d(dst + a.off_wgt, &a.tm_wgt[smp], i0, 0, bar);
         if (++st == stages) {
@@ -243,19 +241,9 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_sweep_lanes(const __grid_c
   for (int j = 0; j < RHO; ++j)
 #pragma unroll
     for (int q = 0; q < NA; ++q) acc[j][q] = 0.0;
-  // Byte offset of (resonance j, helicity h, this lane's event) inside a sub-tile for the first EW-event column of
-  // the sub-tile: plane row * 128 + ((e ^ (row & 7)) << 4)  (128-byte swizzle: the 16-byte chunk index is XORed with
-  // the row index modulo 8).  The column's chunk base cb (a multiple of EW) enters as one more XOR: (cb + e) ^ x
-  // = cb ^ (e ^ x).
-  static_assert(EW <= SUB, "a pass must not span sub-tiles");
-  unsigned foff[RHO][H];
-#pragma unroll
-  for (int j = 0; j < RHO; ++j)
-#pragma unroll
-    for (int h = 0; h < H; ++h) {
-      const unsigned row = (unsigned)((j * SW + s) * H + h);
-      foff[j][h] = row * (SUB * 16) + (((unsigned)e ^ (row & 7u)) << 4);
-    }
+  // byte offset of (resonance 0 of this slice, helicity 0, this lane's event in column 0) inside a stage; resonance j,
+  // helicity h and the column add compile-time / warp-uniform constants
+  const unsigned lane_f = (unsigned)s * (H * TILE * 16) + (unsigned)e * 16u;
   const double* lane_k = Ks + s * KS;
 
   // pass g = w + k NW  ->  local tile t = g / NP, column col = g % NP
@@ -274,8 +262,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_sweep_lanes(const __grid_c
       mbar_wait(full0 + 8 * st, (uint32_t)ph);
       const unsigned char* sp = smem_raw + (size_t)st * a.stage_bytes;
       // sub-tile of this column and the XOR term of its chunk base
-      const unsigned char* fp = sp + (unsigned)((col * EW) / SUB) * a.sub_bytes;
-      const unsigned cbx = (unsigned)((col * EW) % SUB) << 4;
+      const unsigned char* fp = sp + lane_f + (col * EW) * 16;
       double wt = 1.0;
       if (weighted) wt = reinterpret_cast<const double*>(sp + a.off_wgt)[ev];
 
@@ -297,7 +284,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_sweep_lanes(const __grid_c
           const double zr = fma(c.x, br, -(c.y * bi)), zi = fma(c.x, bi, c.y * br);
 #pragma unroll
           for (int h = 0; h < H; ++h) {
-            const double2 F = *reinterpret_cast<const double2*>(fp + (foff[j][h] ^ cbx));
+            const double2 F = *reinterpret_cast<const double2*>(fp + (j * SW * H + h) * (TILE * 16));
             if (j == 0) {
               x[2 * h] = fma(zr, F.x, -(zi * F.y));
               x[2 * h + 1] = fma(zr, F.y, zi * F.x);
@@ -315,7 +302,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_sweep_lanes(const __grid_c
           }
 #pragma unroll
           for (int h = 0; h < H; ++h) {
-            const double2 F = *reinterpret_cast<const double2*>(fp + (foff[j][h] ^ cbx));
+            const double2 F = *reinterpret_cast<const double2*>(fp + (j * SW * H + h) * (TILE * 16));
             const double gx = fma(br, F.x, -(bi * F.y)), gy = fma(br, F.y, bi * F.x);
             Gr[j][h] = make_double2(gx, gy);
             if (j == 0) {

@@ -1,0 +1,34 @@
+// pwa_sweep_lanes_inst.cu - instantiates the lanes sweep kernel for ONE helicity count (-DPWA_LANES_H=1..4), so that
+// the four counts compile in parallel (build.py).  The (RHO, LOG_SW, NW) table must match kLanesCombos in pwa_internal.h.
+#include "pwa_internal.h"
+
+#ifndef PWA_LANES_H
+#error "compile with -DPWA_LANES_H=<n_hel>"
+#endif
+
+namespace pwa {
+namespace {
+template <int RHO, int LOG_SW, int NW>
+lanes_fn for_mode(int mode) {
+  switch (mode) {
+    case MODE_NLL: return lanes::k_sweep_lanes<PWA_LANES_H, RHO, LOG_SW, NW, MODE_NLL>;
+    case MODE_GRAD: return lanes::k_sweep_lanes<PWA_LANES_H, RHO, LOG_SW, NW, MODE_GRAD>;
+    default: return lanes::k_sweep_lanes<PWA_LANES_H, RHO, LOG_SW, NW, MODE_FULL>;
+  }
+}
+}  // namespace
+
+#define PWA_CAT2(a, b) a##b
+#define PWA_CAT(a, b) PWA_CAT2(a, b)
+lanes_fn PWA_CAT(lanes_kernel_h, PWA_LANES_H)(int combo, int mode) {
+  switch (combo) {
+    case 0: return for_mode<1, 2, 15>(mode);
+    case 1: return for_mode<2, 3, 15>(mode);
+    case 2: return for_mode<3, 2, 11>(mode);
+    case 3: return for_mode<4, 3, 7>(mode);
+    case 4: return for_mode<4, 4, 7>(mode);
+    case 5: return for_mode<4, 5, 7>(mode);
+  }
+  return nullptr;
+}
+}  // namespace pwa
