@@ -59,10 +59,10 @@ bool encode_2d(CUtensorMap* m, const void* base, unsigned long long cols, unsign
 // pwa_sweep_lanes.cu
 typedef void (*lanes_fn)(const LaneArgs);
 struct LanesCombo {
-  int rho, log_sw, nw;  // resonances per lane, log2(slices per warp), compute warps per block
+  int rho, log_sw, nw, prod;  // resonances per lane, log2(slices per warp), compute warps per block, producer kind (0 warp, 2 warpgroup)
 };
 // instantiated (RHO, LOG_SW, NW) triples (pwa_sweep_lanes_inst.cu); capacity RHO << LOG_SW resonances
-constexpr LanesCombo kLanesCombos[] = {{1, 2, 15}, {2, 3, 15}, {3, 2, 11}, {4, 3, 7}, {4, 4, 7}, {4, 5, 7}};
+constexpr LanesCombo kLanesCombos[] = {{1, 2, 15, 0}, {2, 3, 15, 0}, {3, 2, 11, 0}, {4, 3, 8, 2}, {4, 3, 7, 0}, {4, 4, 7, 0}, {4, 5, 7, 0}};
 constexpr int kNumLanesCombos = sizeof(kLanesCombos) / sizeof(kLanesCombos[0]);
 lanes_fn lanes_kernel_h1(int combo, int mode);
 lanes_fn lanes_kernel_h2(int combo, int mode);

@@ -79,6 +79,7 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
     return PWA_OK;
   }
   const int rho = kLanesCombos[combo].rho, log_sw = kLanesCombos[combo].log_sw, nw = kLanesCombos[combo].nw;
+  const int prod = kLanesCombos[combo].prod, nthreads = lanes::lanes_threads(nw, prod);
   const int SW = 1 << log_sw, RP = rho * SW, NW = nw;
 
   // amplitude rows incl. the zero-filled planes of padding resonances, in nbox boxes of rows_box (<= 256) rows
@@ -89,7 +90,8 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
   const unsigned stage_bytes = up(off_wgt + lanes::TILE * 8, 128);
   const unsigned k_bytes = up((unsigned)RP * lanes::KS * 8, 128);
   const unsigned red_bytes = up((unsigned)NW * (R * 10 + 2) * 8, 128);
-  const unsigned fixed = k_bytes + red_bytes + 8u * 2 * 8 + 128;
+  const unsigned xch_bytes = up((unsigned)NW * (32 / SW) * 4 * H * 8, 128);
+  const unsigned fixed = k_bytes + red_bytes + xch_bytes + 8u * 2 * 8 + 128;
   int dev_smem = 0;
   cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device);
   int stages = (int)std::min<long long>(8, ((long long)dev_smem - fixed) / stage_bytes);
@@ -103,7 +105,7 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
     cudaError_t ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, dev_smem);
     if (ce != cudaSuccess) return set_error(h, PWA_ERR_CUDA, "cudaFuncSetAttribute(lanes sweep)", ce);
     int occ = 0;
-    ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, (NW + 1) * 32, smem);
+    ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, nthreads, smem);
     if (ce != cudaSuccess || occ < 1) {
       cudaGetLastError();
       why = "lanes kernel cannot be resident (registers / shared memory)";
@@ -127,17 +129,19 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
   }
   a.ch = h->d_ch;
   a.R = R; a.C = C; a.stages = stages;
+  a.dbg = env_int("PWA_DEBUG", 0);
   a.nbox = nbox; a.rows_box = rows_box;
   a.stage_bytes = stage_bytes; a.amp_bytes = amp_bytes; a.off_mass = off_mass; a.off_wgt = off_wgt;
   a.off_K = (unsigned)stages * stage_bytes;
   a.off_red = a.off_K + k_bytes;
-  a.off_bar = a.off_red + red_bytes;
+  a.off_xch = a.off_red + red_bytes;
+  a.off_bar = a.off_xch + xch_bytes;
   h->lanes_smem = smem;
   h->lanes_combo = combo;
   h->variant = 2;
-  h->block = (NW + 1) * 32;
+  h->block = nthreads;
   h->grid = h->num_sms;
-  std::snprintf(h->variant_name, sizeof(h->variant_name), "lanes(rho=%d,sw=%d,nw=%d,stages=%d)", rho, SW, NW, stages);
+  std::snprintf(h->variant_name, sizeof(h->variant_name), "lanes(rho=%d,sw=%d,nw=%d%s,stages=%d)", rho, SW, NW, prod == 2 ? "g" : "", stages);
   return PWA_OK;
 }
 

@@ -37,9 +37,10 @@ struct alignas(64) LaneArgs {
   const int* ch;
   double* partial;  // [2][gridDim.x][R*NACC + 2]
   int R, C, stages;
+  int dbg;  // PWA_DEBUG bit 0: no TMA traffic, compute on whatever the stages hold (timing experiments only)
   int nbox, rows_box;                       // amplitude rows are loaded in nbox boxes of rows_box rows (<= 256)
   unsigned stage_bytes, amp_bytes, off_mass, off_wgt;  // inside a stage: amplitude planes [rows][32 events], mass, weights
-  unsigned off_K, off_red, off_bar;         // after the stages
+  unsigned off_K, off_red, off_bar, off_xch;  // after the stages; xch: [NW][32/SW events][4H] doubles
 };
 
 namespace lanes {
@@ -69,6 +70,20 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "}\n" ::"r"(bar),
       "r"(parity)
       : "memory");
+}
+// non-blocking probe of a phase (acquire): true once the phase with this parity has completed
+__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+      "selp.u32 %0, 1, 0, p;\n"
+      "}\n"
+      : "=r"(ok)
+      : "r"(bar), "r"(parity)
+      : "memory");
+  return ok != 0;
 }
 // TMA tensor copy global -> shared, completion counted in bytes on an mbarrier (SASS: UTMALDG)
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar) {
@@ -124,6 +139,36 @@ __device__ __forceinline__ void slice_allreduce(double (&v)[N], int lane) {
   }
 }
 
+// First half of the exchange: reduce-scatter of v[0..N) over the slice bits MASK, 2 MASK, ..., 16 of the lane id
+// (even N: each half of a lane pair keeps half of the values; odd N: butterfly), then every lane stores the totals
+// it ends up with at their component index in dst (this event's row of the warp's exchange buffer).  The second
+// half is a plain 128-bit read of the row after __syncwarp(): 1 STS + NV/2 LDS instead of NV - 1 shuffles with
+// two selects each.  The order of additions is fixed.
+template <int N, int MASK>
+__device__ __forceinline__ void slice_reduce_store(double (&v)[N], int lane, double* dst) {
+  if constexpr (MASK <= 16) {
+    if constexpr (N % 2 == 0) {
+      constexpr int HF = N / 2;
+      const bool up = (lane & MASK) != 0;
+      double keep[HF];
+#pragma unroll
+      for (int i = 0; i < HF; ++i) {
+        const double send = up ? v[i] : v[i + HF];
+        const double mine = up ? v[i + HF] : v[i];
+        keep[i] = mine + shfl_x(send, MASK);
+      }
+      slice_reduce_store<HF, MASK * 2>(keep, lane, dst + (up ? HF : 0));
+    } else {
+#pragma unroll
+      for (int i = 0; i < N; ++i) v[i] += shfl_x(v[i], MASK);
+      slice_reduce_store<N, MASK * 2>(v, lane, dst);
+    }
+  } else {
+#pragma unroll
+    for (int i = 0; i < N; ++i) dst[i] = v[i];
+  }
+}
+
 // per-resonance constants, packed in pairs for 128-bit shared loads:
 //   k[0..1] = M^2, (M Gamma)^2   k[2] = M Gamma   k[3] = bits: byte offset of the resonance's mass row in a stage
 //   k[4..5] = c   k[6..7] = alpha   k[8..9] = beta          (definitions: pwa_common.cuh)
@@ -161,8 +206,15 @@ __host__ __device__ constexpr int nacc_of() {
 // so NW = 7 / 11 / 15 allows 255 / 168 / 128 registers per thread.
 
 // ------------------------------------------------------------------------------------------------------
-template <int H, int RHO, int LOG_SW, int NW, int MODE>
-__global__ void __launch_bounds__((NW + 1) * 32, 1) k_sweep_lanes(const __grid_constant__ LaneArgs a) {
+// PROD selects who feeds the ring:
+//   0  warp NW is a dedicated producer (NW + 1 warps; with NW = 7 one SM sub-partition has a single compute warp);
+//      (a variant without any producer warp, the compute warp of column 0 issuing the copies, was measured slower:
+//      the feed then waits for that warp's turn);
+//   2  producer warpgroup: warps 0..3 shrink to 24 registers (setmaxnreg.dec), warp 0 produces; the NW compute warps
+//      4..NW+3 grow to 240 registers (setmaxnreg.inc), so every sub-partition carries NW / 4 compute warps.
+constexpr int lanes_threads(int nw, int prod) { return (nw + (prod == 2 ? 4 : 1)) * 32; }
+template <int H, int RHO, int LOG_SW, int NW, int MODE, int PROD>
+__global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(const __grid_constant__ LaneArgs a) {
   constexpr int SW = 1 << LOG_SW;          // slices per warp
   constexpr int EW = 32 / SW;              // events per pass
   constexpr int NP = SW;                   // passes per tile
@@ -171,7 +223,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_sweep_lanes(const __grid_c
   constexpr int NA = NACC > 0 ? NACC : 1;
   constexpr int RP = RHO * SW;             // resonances incl. padding
   extern __shared__ __align__(1024) unsigned char smem_raw[];
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31, w = (int)(threadIdx.x >> 5) - (PROD == 2 ? 4 : 0);  // w: compute-warp index
   const int R = a.R, stages = a.stages;
   double* Ks = reinterpret_cast<double*>(smem_raw + a.off_K);    // [RP][KS]
   double* red = reinterpret_cast<double*>(smem_raw + a.off_red);  // [NW][R*NACC + 2]
@@ -204,36 +256,37 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_sweep_lanes(const __grid_c
   const int TdB = b < tilesD ? (tilesD - b + G - 1) / G : 0;
   const int T = TmB + TdB;
 
-  // ======================================= producer warp ===================================================
-  if (w == NW) {
-    if (lane == 0) {
+  // ======================================= producer ========================================================
+  // copies of local tile k into its stage; the caller has made sure the stage is free
+  auto issue_tile = [&](int k) {
+    const int smp = k >= TmB ? 1 : 0;
+    const int i0 = (b + (k - (smp ? TmB : 0)) * G) * TILE;
+    const bool wg = smp == 1 && a.weighted;
+    const int st = k % stages;
+    const uint32_t bar = full0 + 8 * st, dst = smem_u32(smem_raw) + st * a.stage_bytes;
+    mbar_expect_tx(bar, a.amp_bytes + (unsigned)a.C * (TILE * 8) + (wg ? TILE * 8u : 0u));
+    for (int x = 0; x < a.nbox; ++x)
+      tma_load_2d(dst + x * a.rows_box * (TILE * 16), &a.tm_amp[smp], 2 * i0, x * a.rows_box, bar);
+    tma_load_2d(dst + a.off_mass, &a.tm_mass[smp], i0, 0, bar);
+    if (wg) tma_load_2d(dst + a.off_wgt, &a.tm_wgt[smp], i0, 0, bar);
+  };
+  if ((PROD == 0 && w == NW) || (PROD == 2 && w < 0)) {
+    if (PROD == 2) asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
+    if (lane == 0 && (PROD == 0 || w == -4) && !(a.dbg & 1)) {
       tma_prefetch_desc(&a.tm_amp[0]);
       tma_prefetch_desc(&a.tm_mass[0]);
       tma_prefetch_desc(&a.tm_amp[1]);
       tma_prefetch_desc(&a.tm_mass[1]);
-      const uint32_t tx = a.amp_bytes + (unsigned)a.C * (TILE * 8);
-      int st = 0, round = 0;
       for (int k = 0; k < T; ++k) {
-        if (round > 0) mbar_wait(empty0 + 8 * st, (uint32_t)((round - 1) & 1));
-        const int smp = k >= TmB ? 1 : 0;
-        const int i0 = (b + (k - (smp ? TmB : 0)) * G) * TILE;
-        const bool wg = smp == 1 && a.weighted;
-        const uint32_t bar = full0 + 8 * st, dst = smem_u32(smem_raw) + st * a.stage_bytes;
-        mbar_expect_tx(bar, tx + (wg ? TILE * 8u : 0u));
-        for (int x = 0; x < a.nbox; ++x)
-          tma_load_2d(dst + x * a.rows_box * (TILE * 16), &a.tm_amp[smp], 2 * i0, x * a.rows_box, bar);
-        tma_load_2d(dst + a.off_mass, &a.tm_mass[smp], i0, 0, bar);
-        if (wg) tma_load_2d(dst + a.off_wgt, &a.tm_wgt[smp], i0, 0, bar);
-        if (++st == stages) {
-          st = 0;
-          ++round;
-        }
+        if (k >= stages) mbar_wait(empty0 + 8 * (k % stages), (uint32_t)((k / stages - 1) & 1));
+        issue_tile(k);
       }
     }
     return;
   }
 
   // ======================================= compute warps ===================================================
+  if (PROD == 2) asm volatile("setmaxnreg.inc.sync.aligned.u32 240;");
   const int s = lane >> (5 - LOG_SW), e = lane & (EW - 1);
   double acc[RHO][NA];
   double s0 = 0.0, s1 = 0.0;
@@ -245,11 +298,33 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_sweep_lanes(const __grid_c
   // helicity h and the column add compile-time / warp-uniform constants
   const unsigned lane_f = (unsigned)s * (H * TILE * 16) + (unsigned)e * 16u;
   const double* lane_k = Ks + s * KS;
+  unsigned moff[RHO];  // byte offset of each own resonance's mass row inside a stage (kept in registers: no dependent load)
+#pragma unroll
+  for (int j = 0; j < RHO; ++j) moff[j] = (unsigned)__double_as_longlong(lane_k[j * (SW * KS) + 3]);
+  double* xrow = reinterpret_cast<double*>(smem_raw + a.off_xch) + ((size_t)w * EW + e) * (4 * H);  // this event's exchange row
 
   // pass g = w + k NW  ->  local tile t = g / NP, column col = g % NP
   int t = w / NP, col = w % NP;
   int st = t % stages, ph = (t / stages) & 1;
 
+  // Propagators of one pass (a-1): B_r = conj(D_r)/|D_r|^2 for this lane's RHO resonances and its event of column
+  // col_ of the tile in stage st_.
+  auto propagators = [&](int st_, int col_, bool valid_, double2 (&Bo)[RHO]) {
+    const unsigned char* sp_ = smem_raw + (size_t)st_ * a.stage_bytes;
+    const int ev_ = col_ * EW + e;
+#pragma unroll
+    for (int j = 0; j < RHO; ++j) {
+      const double2* kk = reinterpret_cast<const double2*>(lane_k + j * (SW * KS));
+      const double2 k01 = kk[0];
+      const double mg = lane_k[j * (SW * KS) + 2];
+      const double m = *reinterpret_cast<const double*>(sp_ + moff[j] + ev_ * 8);
+      const double xx = fma(-m, m, k01.x);
+      double den = fma(xx, xx, k01.y);
+      den = valid_ ? den : 1.0;  // lanes beyond the ragged end stay finite
+      const double u = fast_rcp(den);
+      Bo[j] = make_double2(xx * u, mg * u);  // B = conj(D)/|D|^2
+    }
+  };
   for (int smp = 0; smp < 2; ++smp) {
     const int t_end = smp ? T : TmB;
     const long long n = smp ? nD : nM;
@@ -259,9 +334,8 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_sweep_lanes(const __grid_c
       const long long i0 = (long long)(b + (t - (smp ? TmB : 0)) * G) * TILE;
       const int ev = col * EW + e;
       const bool valid = i0 + ev < n;
-      mbar_wait(full0 + 8 * st, (uint32_t)ph);
+      if (!(a.dbg & 1)) mbar_wait(full0 + 8 * st, (uint32_t)ph);
       const unsigned char* sp = smem_raw + (size_t)st * a.stage_bytes;
-      // sub-tile of this column and the XOR term of its chunk base
       const unsigned char* fp = sp + lane_f + (col * EW) * 16;
       double wt = 1.0;
       if (weighted) wt = reinterpret_cast<const double*>(sp + a.off_wgt)[ev];
@@ -269,17 +343,12 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_sweep_lanes(const __grid_c
       // ---------------- forward ----------------
       double2 Gr[RHO][H], Br[RHO];
       double x[NV];  // slice partials: A_h (re, im) [then Adot_h (re, im)]
+      propagators(st, col, valid, Br);
 #pragma unroll
       for (int j = 0; j < RHO; ++j) {
         const double2* kk = reinterpret_cast<const double2*>(lane_k + j * (SW * KS));
-        const double2 k01 = kk[0], k23 = kk[1], c = kk[2];
-        const double m = *reinterpret_cast<const double*>(sp + (unsigned)__double_as_longlong(k23.y) + ev * 8);
-        const double xx = fma(-m, m, k01.x);
-        double den = fma(xx, xx, k01.y);
-        den = valid ? den : 1.0;  // lanes beyond the ragged end stay finite
-        const double u = fast_rcp(den);
-        const double br = xx * u, bi = k23.x * u;  // B = conj(D)/|D|^2
-        Br[j] = make_double2(br, bi);
+        const double2 c = kk[2];
+        const double br = Br[j].x, bi = Br[j].y;
         if (MODE == MODE_NLL) {
           const double zr = fma(c.x, br, -(c.y * bi)), zi = fma(c.x, bi, c.y * br);
 #pragma unroll
@@ -328,7 +397,14 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_sweep_lanes(const __grid_c
       if (lane == 0) mbar_arrive(empty0 + 8 * st);
 
       // ---------------- exchange over the slices ----------------
-      slice_allreduce<NV, EW>(x, lane);
+      slice_reduce_store<NV, EW>(x, lane, xrow);
+      __syncwarp();
+#pragma unroll
+      for (int i = 0; i < NV; i += 2) {
+        const double2 p = *reinterpret_cast<const double2*>(xrow + i);
+        x[i] = p.x;
+        x[i + 1] = p.y;
+      }
 
       // ---------------- event: I, and for data ln I, omega, kappa ----------------
       double I = 0.0;
@@ -451,7 +527,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_sweep_lanes(const __grid_c
     }
     asm volatile("bar.sync 1, %0;" ::"n"(NW * 32) : "memory");
     double* out = a.partial + ((size_t)smp * gridDim.x + blockIdx.x) * (size_t)row_len;
-    for (int k = threadIdx.x; k < row_len; k += NW * 32) {
+    for (int k = w * 32 + lane; k < row_len; k += NW * 32) {
       double tsum = red[k];
       for (int ww = 1; ww < NW; ++ww) tsum += red[(size_t)ww * row_len + k];
       out[k] = tsum;

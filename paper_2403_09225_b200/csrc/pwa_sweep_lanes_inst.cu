@@ -8,12 +8,12 @@
 
 namespace pwa {
 namespace {
-template <int RHO, int LOG_SW, int NW>
+template <int RHO, int LOG_SW, int NW, int PROD = 0>
 lanes_fn for_mode(int mode) {
   switch (mode) {
-    case MODE_NLL: return lanes::k_sweep_lanes<PWA_LANES_H, RHO, LOG_SW, NW, MODE_NLL>;
-    case MODE_GRAD: return lanes::k_sweep_lanes<PWA_LANES_H, RHO, LOG_SW, NW, MODE_GRAD>;
-    default: return lanes::k_sweep_lanes<PWA_LANES_H, RHO, LOG_SW, NW, MODE_FULL>;
+    case MODE_NLL: return lanes::k_sweep_lanes<PWA_LANES_H, RHO, LOG_SW, NW, MODE_NLL, PROD>;
+    case MODE_GRAD: return lanes::k_sweep_lanes<PWA_LANES_H, RHO, LOG_SW, NW, MODE_GRAD, PROD>;
+    default: return lanes::k_sweep_lanes<PWA_LANES_H, RHO, LOG_SW, NW, MODE_FULL, PROD>;
   }
 }
 }  // namespace
@@ -25,9 +25,10 @@ lanes_fn PWA_CAT(lanes_kernel_h, PWA_LANES_H)(int combo, int mode) {
     case 0: return for_mode<1, 2, 15>(mode);
     case 1: return for_mode<2, 3, 15>(mode);
     case 2: return for_mode<3, 2, 11>(mode);
-    case 3: return for_mode<4, 3, 7>(mode);
-    case 4: return for_mode<4, 4, 7>(mode);
-    case 5: return for_mode<4, 5, 7>(mode);
+    case 3: return for_mode<4, 3, 8, 2>(mode);
+    case 4: return for_mode<4, 3, 7>(mode);
+    case 5: return for_mode<4, 4, 7>(mode);
+    case 6: return for_mode<4, 5, 7>(mode);
   }
   return nullptr;
 }
