@@ -301,6 +301,20 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
   unsigned moff[RHO];  // byte offset of each own resonance's mass row inside a stage (kept in registers: no dependent load)
 #pragma unroll
   for (int j = 0; j < RHO; ++j) moff[j] = (unsigned)__double_as_longlong(lane_k[j * (SW * KS) + 3]);
+  // with the producer warpgroup the compute warps own 240 registers: keep the constants every pass needs in
+  // registers instead of re-reading them from shared memory (one wavefront per 4 bytes per lane, broadcast or not)
+  constexpr bool KREG = PROD == 2;
+  double2 creg[RHO], k01reg[RHO];
+  double mgreg[RHO];
+  if (KREG) {
+#pragma unroll
+    for (int j = 0; j < RHO; ++j) {
+      const double2* kk = reinterpret_cast<const double2*>(lane_k + j * (SW * KS));
+      k01reg[j] = kk[0];
+      mgreg[j] = lane_k[j * (SW * KS) + 2];
+      creg[j] = kk[2];
+    }
+  }
   double* xrow = reinterpret_cast<double*>(smem_raw + a.off_xch) + ((size_t)w * EW + e) * (4 * H);  // this event's exchange row
 
   // pass g = w + k NW  ->  local tile t = g / NP, column col = g % NP
@@ -315,8 +329,8 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
 #pragma unroll
     for (int j = 0; j < RHO; ++j) {
       const double2* kk = reinterpret_cast<const double2*>(lane_k + j * (SW * KS));
-      const double2 k01 = kk[0];
-      const double mg = lane_k[j * (SW * KS) + 2];
+      const double2 k01 = KREG ? k01reg[j] : kk[0];
+      const double mg = KREG ? mgreg[j] : lane_k[j * (SW * KS) + 2];
       const double m = *reinterpret_cast<const double*>(sp_ + moff[j] + ev_ * 8);
       const double xx = fma(-m, m, k01.x);
       double den = fma(xx, xx, k01.y);
@@ -347,7 +361,7 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
 #pragma unroll
       for (int j = 0; j < RHO; ++j) {
         const double2* kk = reinterpret_cast<const double2*>(lane_k + j * (SW * KS));
-        const double2 c = kk[2];
+        const double2 c = KREG ? creg[j] : kk[2];
         const double br = Br[j].x, bi = Br[j].y;
         if (MODE == MODE_NLL) {
           const double zr = fma(c.x, br, -(c.y * bi)), zi = fma(c.x, bi, c.y * br);
