@@ -141,9 +141,11 @@ def _dev_f64(t, n, name):
 # ---- the C calls, one to one ------------------------------------------------------------------------------
 def pwa_create(res_chan, data_mass, data_amp, data_weight, mc_mass, mc_amp, *, borrow: bool = False, device: int = 0,
                stream: int = 0, data_stride: int = 0, mc_stride: int = 0, n_data: Optional[int] = None,
-               n_mc: Optional[int] = None) -> int:
+               n_mc: Optional[int] = None, data_first: int = 0, mc_first: int = 0) -> int:
     """Creates a handle from torch tensors (CPU or CUDA, float64, contiguous) in the layouts of pwa.h:
-    mass [C][N], amp [R][H][N][2], weight [N] or None, res_chan [R] int32 (CPU).  Returns the handle."""
+    mass [C][N], amp [R][H][N][2], weight [N] or None, res_chan [R] int32 (CPU).  Returns the handle.
+    A window of a larger store (an event shard) is described without copying by `*_first` (first
+    event), `n_*` (event count) and `*_stride` (events between planes of the full store)."""
     import torch
     lib = load()
     tensors = [data_mass, data_amp, mc_mass, mc_amp] + ([data_weight] if data_weight is not None else [])
@@ -159,10 +161,15 @@ def pwa_create(res_chan, data_mass, data_amp, data_weight, mc_mass, mc_amp, *, b
     d = pwa_model_desc()
     d.n_res, d.n_hel, d.n_chan = R, H, C
     d.res_chan = rc.data_ptr()
-    d.data = pwa_sample(int(data_mass.shape[1]) if n_data is None else n_data, data_stride,
-                        data_mass.data_ptr(), data_amp.data_ptr(), _ptr(data_weight))
-    d.mc = pwa_sample(int(mc_mass.shape[1]) if n_mc is None else n_mc, mc_stride, mc_mass.data_ptr(),
-                      mc_amp.data_ptr(), None)
+    if (data_first or n_data is not None) and not data_stride:
+        data_stride = int(data_mass.shape[1])
+    if (mc_first or n_mc is not None) and not mc_stride:
+        mc_stride = int(mc_mass.shape[1])
+    d.data = pwa_sample(int(data_mass.shape[1]) - data_first if n_data is None else n_data, data_stride,
+                        data_mass.data_ptr() + 8 * data_first, data_amp.data_ptr() + 16 * data_first,
+                        None if data_weight is None else data_weight.data_ptr() + 8 * data_first)
+    d.mc = pwa_sample(int(mc_mass.shape[1]) - mc_first if n_mc is None else n_mc, mc_stride,
+                      mc_mass.data_ptr() + 8 * mc_first, mc_amp.data_ptr() + 16 * mc_first, None)
     d.mem = PWA_MEM_DEVICE if on_dev.pop() else PWA_MEM_HOST
     d.borrow = 1 if borrow else 0
     d.device = device

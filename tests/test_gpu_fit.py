@@ -1,0 +1,93 @@
+"""GPU fit (pwa_fit_newton_cg, a-8) against the reference fit oracle/fit.py (S15/S19).
+
+The fit is an iteration whose end point is not unique (S14: global phase, common scale, local minima), so
+raw theta is never compared.  What is unique and compared:
+  * from the same start, with the same options, both sides run the same algorithm: the NLL reached agrees to
+    1e-7 relative, the convergence classification is the same, and the sweep counts agree closely (rounding may
+    shift a CG exit by an iteration);
+  * at the point the CUDA fit returns, the ORACLE's gradient is small and its NLL equals the reported one
+    (north_star tolerances): the result is checked by the oracle, not by the kernel that produced it;
+  * the NLL never increased (Armijo) and the S19 box holds at the returned point;
+  * a start with a non-finite NLL (all couplings zero: ln 0) is reported as PWA_ERR_NONFINITE.
+"""
+import numpy as np
+import pytest
+import torch
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def setup(oracle_mod):
+    import paper_2403_09225_b200 as pwa
+    import workloads
+    from paper_2403_09225_b200.build import build
+    build()
+    pwa.load()
+    assert torch.cuda.is_available(), "the gpu tests need a CUDA device"
+    out = {}
+    for idx, n_mc, n_data in ((1, 20_000, 4_000), (2, 30_000, 3_000)):
+        cfg = workloads.CONFIGS[idx].scaled(n_mc, n_data)
+        w = workloads.make_workload(cfg, "cpu", chunk=1 << 13, imax_events=n_mc)
+        out[idx] = (cfg, w, oracle_mod.model_from_workload(w), pwa.Model(w))
+    return pwa, workloads, out
+
+
+def _opts(pwa, **kw):
+    o = pwa.pwa_fit_opts_default()
+    for k, v in kw.items():
+        setattr(o, k, v)
+    return o
+
+
+@pytest.mark.parametrize("idx", [1, 2])
+def test_fit_from_theta_true_matches_the_reference_fit(oracle_mod, setup, idx):
+    from oracle.fit import FitOpts, fit_newton_cg
+    pwa, workloads, models = setup
+    cfg, w, om, gm = models[idx]
+    th0 = workloads.theta_true(cfg).numpy()
+    ref = fit_newton_cg(om, th0, FitOpts(), prec="d", threads=oracle_mod.max_threads())
+    th, res = gm.fit(th0)
+    assert ref.converged and res.status == 0, (ref.stop_reason, res.stop_reason, res.status)
+    assert res.stop_reason in (1, 2, 3)
+    assert abs(res.nll - ref.nll) <= 1e-7 * max(1.0, abs(ref.nll)), (res.nll, ref.nll)
+    assert abs(res.outer_iters - ref.outer_iters) <= max(2, ref.outer_iters // 5)
+    assert abs(res.n_hvp - ref.n_hvp) <= max(5, ref.n_hvp // 4)
+    # the oracle's verdict on the point the CUDA fit returned
+    f0, g0, _ = oracle_mod.nll_grad_hvp(om, th, None, "ld")
+    assert abs(float(f0) - res.nll) <= 1e-10 * max(1.0, abs(float(f0)))
+    assert float(np.max(np.abs(np.asarray(g0, dtype=np.float64)))) <= max(10 * res.grad_inf_norm, 1e-3)
+    assert res.nll < float(oracle_mod.nll(om, th0, "d"))
+    o = FitOpts()
+    assert np.all(th[3::4] >= o.gamma_min) and np.all(th[3::4] <= o.gamma_max)
+    assert np.all(th[2::4] >= o.mass_min) and np.all(th[2::4] <= o.mass_max)
+    assert res.n_grad >= res.outer_iters and res.n_hvp == res.cg_iters and res.seconds > 0.0
+
+
+def test_fit_from_random_starts_follows_the_reference(oracle_mod, setup):
+    """Random starts (S16) wander through many iterations; with a short budget both sides must have descended
+    to nearly the same NLL, and the CUDA value must be the oracle's NLL at the returned point."""
+    from oracle.fit import FitOpts, fit_newton_cg
+    pwa, workloads, models = setup
+    cfg, w, om, gm = models[1]
+    for k in range(3):
+        th0 = workloads.random_start(cfg, k).numpy()
+        ref = fit_newton_cg(om, th0, FitOpts(max_outer=6), prec="d", threads=oracle_mod.max_threads())
+        th, res = gm.fit(th0, _opts(pwa, max_outer=6))
+        f_start = float(oracle_mod.nll(om, th0, "d"))
+        assert res.nll <= f_start and ref.nll <= f_start
+        assert abs(res.nll - ref.nll) <= 1e-6 * max(1.0, abs(ref.nll)), (k, res.nll, ref.nll)
+        assert res.outer_iters == ref.outer_iters and res.stop_reason == ref.stop_reason
+        f0 = float(oracle_mod.nll(om, th, "ld"))
+        assert abs(f0 - res.nll) <= 1e-10 * max(1.0, abs(f0))
+
+
+def test_nonfinite_start_is_reported(setup):
+    pwa, workloads, models = setup
+    cfg, w, om, gm = models[1]
+    th0 = workloads.theta_true(cfg).numpy().copy()
+    th0[0::4] = 0.0  # all couplings zero: I = 0 on every event, ln I = -inf (S8)
+    th, res = gm.fit(th0)
+    assert res.status == 4  # PWA_ERR_NONFINITE, reported in the result, theta left at the start point
+    assert np.array_equal(th, th0)
+    assert pwa.pwa_status_flags(gm.h) & 1
