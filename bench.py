@@ -261,13 +261,15 @@ def main():
     sweep_avg_s = (sweep_ms / max(sweep_n, 1)) * 1e-3
     achieved = bytes_per_step / sweep_avg_s / 1e9 if sweep_n else None
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")  # ncu dram bytes per sweep launch, written from a capture
+    # ncu dram__bytes_read.sum + dram__bytes_write.sum per sweep launch, copied from the committed --set full capture
+    tpath = os.path.join(ROOT, "profiles", "r01_traffic.csv")  # columns: config,kernel_variant,dram_bytes_per_launch
     if os.path.exists(tpath):
         try:
             with open(tpath) as f:
-                tj = json.load(f)
-            key = f"config{args.config}:{pwa.pwa_kernel_variant(m.h)}"
-            traffic = tj.get(key)
+                for row in f:
+                    parts = [x.strip() for x in row.strip().split(";")]
+                    if len(parts) == 3 and parts[0] == f"config{args.config}" and parts[1] == pwa.pwa_kernel_variant(m.h):
+                        traffic = float(parts[2])
         except Exception:
             traffic = None
     line = {
