@@ -129,7 +129,6 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
   }
   a.ch = h->d_ch;
   a.R = R; a.C = C; a.stages = stages;
-  a.dbg = env_int("PWA_DEBUG", 0);
   a.nbox = nbox; a.rows_box = rows_box;
   a.stage_bytes = stage_bytes; a.amp_bytes = amp_bytes; a.off_mass = off_mass; a.off_wgt = off_wgt;
   a.off_K = (unsigned)stages * stage_bytes;

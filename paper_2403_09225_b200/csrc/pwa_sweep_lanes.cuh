@@ -37,7 +37,6 @@ struct alignas(64) LaneArgs {
   const int* ch;
   double* partial;  // [2][gridDim.x][R*NACC + 2]
   int R, C, stages;
-  int dbg;  // PWA_DEBUG bit 0: no TMA traffic, compute on whatever the stages hold (timing experiments only)
   int nbox, rows_box;                       // amplitude rows are loaded in nbox boxes of rows_box rows (<= 256)
   unsigned stage_bytes, amp_bytes, off_mass, off_wgt;  // inside a stage: amplitude planes [rows][32 events], mass, weights
   unsigned off_K, off_red, off_bar, off_xch;  // after the stages; xch: [NW][32/SW events][4H] doubles
@@ -46,6 +45,11 @@ struct alignas(64) LaneArgs {
 namespace lanes {
 
 constexpr int TILE = 32;       // events per tile
+#ifdef PWA_DEBUG_NOLOAD           // timing experiments only: no TMA traffic, compute on whatever the stages hold
+constexpr bool kNoLoad = true;
+#else
+constexpr bool kNoLoad = false;
+#endif
 constexpr int KS = 10;         // doubles of constants per resonance
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -272,7 +276,7 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
   };
   if ((PROD == 0 && w == NW) || (PROD == 2 && w < 0)) {
     if (PROD == 2) asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
-    if (lane == 0 && (PROD == 0 || w == -4) && !(a.dbg & 1)) {
+    if (lane == 0 && (PROD == 0 || w == -4) && !kNoLoad) {
       tma_prefetch_desc(&a.tm_amp[0]);
       tma_prefetch_desc(&a.tm_mass[0]);
       tma_prefetch_desc(&a.tm_amp[1]);
@@ -341,14 +345,14 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
   };
   for (int smp = 0; smp < 2; ++smp) {
     const int t_end = smp ? T : TmB;
-    const long long n = smp ? nD : nM;
+    const int n = (int)(smp ? nD : nM);
     const bool weighted = smp == 1 && a.weighted;
 #pragma unroll 1
     while (t < t_end) {
-      const long long i0 = (long long)(b + (t - (smp ? TmB : 0)) * G) * TILE;
+      const int i0 = (b + (t - (smp ? TmB : 0)) * G) * TILE;  // < 2^30 (lanes_configure)
       const int ev = col * EW + e;
       const bool valid = i0 + ev < n;
-      if (!(a.dbg & 1)) mbar_wait(full0 + 8 * st, (uint32_t)ph);
+      if (!kNoLoad) mbar_wait(full0 + 8 * st, (uint32_t)ph);
       const unsigned char* sp = smem_raw + (size_t)st * a.stage_bytes;
       const unsigned char* fp = sp + lane_f + (col * EW) * 16;
       double wt = 1.0;
