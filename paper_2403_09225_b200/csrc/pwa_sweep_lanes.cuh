@@ -185,6 +185,9 @@ __device__ __forceinline__ void resonance_constants(const double* __restrict__ t
   const cplx cc = {a * c, a * s};
   k[0] = M * M;
   k[1] = (M * G) * (M * G);
+  // Events beyond the ragged end read zero-filled masses and amplitudes: |D|^2 = M^4 + (M Gamma)^2 there.  A resonance
+  // with M = 0 exactly would give 1/0 * 0 = NaN on those lanes; a denominator floor far below any m^4 keeps them at 0.
+  if (k[0] == 0.0 && k[1] == 0.0) k[1] = 1e-300;
   k[2] = M * G;
   k[3] = __longlong_as_double(mass_off);
   k[4] = cc.re;
@@ -327,7 +330,7 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
 
   // Propagators of one pass (a-1): B_r = conj(D_r)/|D_r|^2 for this lane's RHO resonances and its event of column
   // col_ of the tile in stage st_.
-  auto propagators = [&](int st_, int col_, bool valid_, double2 (&Bo)[RHO]) {
+  auto propagators = [&](int st_, int col_, double2 (&Bo)[RHO]) {
     const unsigned char* sp_ = smem_raw + (size_t)st_ * a.stage_bytes;
     const int ev_ = col_ * EW + e;
 #pragma unroll
@@ -337,8 +340,7 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
       const double mg = KREG ? mgreg[j] : lane_k[j * (SW * KS) + 2];
       const double m = *reinterpret_cast<const double*>(sp_ + moff[j] + ev_ * 8);
       const double xx = fma(-m, m, k01.x);
-      double den = fma(xx, xx, k01.y);
-      den = valid_ ? den : 1.0;  // lanes beyond the ragged end stay finite
+      const double den = fma(xx, xx, k01.y);  // > 0 also on the zero-filled lanes beyond the ragged end
       const double u = fast_rcp(den);
       Bo[j] = make_double2(xx * u, mg * u);  // B = conj(D)/|D|^2
     }
@@ -361,7 +363,7 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
       // ---------------- forward ----------------
       double2 Gr[RHO][H], Br[RHO];
       double x[NV];  // slice partials: A_h (re, im) [then Adot_h (re, im)]
-      propagators(st, col, valid, Br);
+      propagators(st, col, Br);
 #pragma unroll
       for (int j = 0; j < RHO; ++j) {
         const double2* kk = reinterpret_cast<const double2*>(lane_k + j * (SW * KS));

@@ -167,3 +167,21 @@ def test_host_entry_point(pwa, oracle_mod):
     pwa.pwa_nll_grad_hvp_host(gm.h, np.ascontiguousarray(th), None, nll, g2, None)
     f0, g0, _ = oracle_mod.nll_grad_hvp(om, th, None, "ld")
     assert _nll_err(nll[0], f0) < NLL_TOL and rel_l2(g2, g0) < VEC_TOL
+
+
+def test_zero_mass_resonance_on_a_ragged_tail(pwa, oracle_mod):
+    """M_r = 0 makes |D|^2 = m^4: finite on every event, but the zero-filled lanes beyond the ragged end of the last
+    tile would see 1/0 without the kernel's denominator floor (pwa_sweep_lanes.cuh, resonance_constants)."""
+    import workloads
+    for case in (CASES[1], CASES[2]):
+        cfg, w, om, gm = _case(pwa, oracle_mod, *case)
+        assert cfg.n_mc % 32 != 0 and cfg.n_data % 32 != 0
+        th = _thetas(cfg)[1].copy()
+        th[2], th[3] = 0.0, 0.0       # resonance 0: M = 0, Gamma = 0
+        th[6] = 0.0                   # resonance 1: M = 0, Gamma > 0
+        v = workloads.direction(cfg, 7).numpy()
+        f0, g0, h0 = oracle_mod.nll_grad_hvp(om, th, v, "ld")
+        f, g, hv = gm.nll_grad_hvp(th, v)
+        assert np.isfinite(f) and np.all(np.isfinite(g)) and np.all(np.isfinite(hv))
+        assert _nll_err(f, f0) < NLL_TOL and rel_l2(g, g0) < VEC_TOL and rel_l2(hv, h0) < VEC_TOL
+        assert pwa.pwa_status_flags(gm.h) == 0
