@@ -62,7 +62,8 @@ struct LanesCombo {
   int rho, log_sw, nw, prod;  // resonances per lane, log2(slices per warp), compute warps per block, producer kind (0 warp, 2 warpgroup)
 };
 // instantiated (RHO, LOG_SW, NW) triples (pwa_sweep_lanes_inst.cu); capacity RHO << LOG_SW resonances
-constexpr LanesCombo kLanesCombos[] = {{1, 2, 15, 0}, {2, 3, 15, 0}, {3, 2, 11, 0}, {4, 3, 8, 2}, {4, 3, 7, 0}, {4, 4, 7, 0}, {4, 5, 7, 0}};
+constexpr LanesCombo kLanesCombos[] = {{1, 2, 15, 0}, {2, 3, 15, 0}, {3, 2, 8, 2}, {3, 2, 11, 0}, {4, 3, 8, 2}, {4, 3, 7, 0},
+                                       {4, 4, 8, 2}, {4, 4, 7, 0}, {4, 5, 8, 2}, {4, 5, 7, 0}};
 constexpr int kNumLanesCombos = sizeof(kLanesCombos) / sizeof(kLanesCombos[0]);
 lanes_fn lanes_kernel_h1(int combo, int mode);
 lanes_fn lanes_kernel_h2(int combo, int mode);

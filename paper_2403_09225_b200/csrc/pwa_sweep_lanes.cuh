@@ -310,7 +310,7 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
   for (int j = 0; j < RHO; ++j) moff[j] = (unsigned)__double_as_longlong(lane_k[j * (SW * KS) + 3]);
   // with the producer warpgroup the compute warps own 240 registers: keep the constants every pass needs in
   // registers instead of re-reading them from shared memory (one wavefront per 4 bytes per lane, broadcast or not)
-  constexpr bool KREG = PROD == 2;
+  constexpr bool KREG = PROD == 2 && RHO * H <= 9;  // beyond that the amplitudes G_rh themselves fill the file
   double2 creg[RHO], k01reg[RHO];
   double mgreg[RHO];
   if (KREG) {
