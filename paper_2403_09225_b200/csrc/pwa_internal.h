@@ -54,16 +54,21 @@ struct pwa_handle {
 
 namespace pwa {
 // fp64 matrix [rows][row_stride_bytes / 8], valid extent (cols, rows), box (box_cols, box_rows); out-of-bounds reads give 0
+bool encode_3d_swz128(CUtensorMap* m, const void* base, const unsigned long long dims[3], const unsigned long long strides_bytes[2],
+                      const unsigned box[3]);
 bool encode_2d(CUtensorMap* m, const void* base, unsigned long long cols, unsigned long long rows,
                unsigned long long row_stride_bytes, unsigned box_cols, unsigned box_rows, bool swizzle128 = false);
 // pwa_sweep_lanes.cu
 typedef void (*lanes_fn)(const LaneArgs);
 struct LanesCombo {
-  int rho, log_sw, nw, prod;  // resonances per lane, log2(slices per warp), compute warps per block, producer kind (0 warp, 2 warpgroup)
+  int rho, log_sw, nw, prod, tile;  // resonances per lane, log2(slices per warp), compute warps per block, producer kind
+                                    // (0 warp, 2 warpgroup), events per tile (32, or 8 with the swizzled layout)
 };
-// instantiated (RHO, LOG_SW, NW) triples (pwa_sweep_lanes_inst.cu); capacity RHO << LOG_SW resonances
-constexpr LanesCombo kLanesCombos[] = {{1, 2, 15, 0}, {2, 3, 15, 0}, {3, 2, 8, 2}, {3, 2, 11, 0}, {4, 3, 8, 2}, {4, 3, 7, 0},
-                                       {4, 4, 8, 2}, {4, 4, 7, 0}, {4, 5, 8, 2}, {4, 5, 7, 0}};
+// instantiated shapes (pwa_sweep_lanes_inst.cu); capacity RHO << LOG_SW resonances; the handle takes the first entry of
+// the smallest capacity >= R whose stages fit in shared memory at least twice
+constexpr LanesCombo kLanesCombos[] = {{1, 2, 15, 0, 32}, {2, 3, 15, 0, 32}, {3, 2, 8, 2, 32}, {3, 2, 11, 0, 32}, {4, 3, 8, 2, 32},
+                                       {4, 3, 7, 0, 32}, {4, 4, 8, 2, 32}, {4, 4, 7, 0, 32}, {4, 5, 8, 2, 32}, {4, 5, 7, 0, 32},
+                                       {4, 4, 8, 2, 8}, {4, 5, 8, 2, 8}};
 constexpr int kNumLanesCombos = sizeof(kLanesCombos) / sizeof(kLanesCombos[0]);
 lanes_fn lanes_kernel_h1(int combo, int mode);
 lanes_fn lanes_kernel_h2(int combo, int mode);

@@ -1,4 +1,5 @@
 // pwa_sweep_lanes.cu - host side of the warp-autonomous sweep: kernel table, shared-memory plan, launch.
+#include <algorithm>
 #include <cstdlib>
 #include <cstring>
 #include <cstdio>
@@ -44,6 +45,18 @@ bool encode_2d(CUtensorMap* m, const void* base, unsigned long long cols, unsign
             CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+bool encode_3d_swz128(CUtensorMap* m, const void* base, const unsigned long long dims[3], const unsigned long long strides_bytes[2],
+                      const unsigned box[3]) {
+  encode_fn fn = get_encode();
+  if (!fn) return false;
+  cuuint64_t d[3] = {dims[0], dims[1], dims[2]};
+  cuuint64_t st[2] = {strides_bytes[0], strides_bytes[1]};
+  cuuint32_t bx[3] = {box[0], box[1], box[2]};
+  cuuint32_t es[3] = {1, 1, 1};
+  return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void*>(base), d, st, bx, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 lanes_fn lanes_kernel(int H, int combo, int mode) {
   if (combo < 0 || combo >= kNumLanesCombos) return nullptr;
   switch (H) {
@@ -65,39 +78,56 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
       return PWA_OK;
     }
   }
-  // smallest padded capacity among the instantiated combos (ties: the earlier entry); PWA_COMBO forces one
-  int combo = env_int("PWA_COMBO", -1);
-  if (combo < 0) {
-    int best = -1;
-    for (int k = 0; k < kNumLanesCombos; ++k) {
-      const int cap = kLanesCombos[k].rho << kLanesCombos[k].log_sw;
-      if (cap >= R && (best < 0 || cap < best)) { best = cap; combo = k; }
-    }
-  }
-  if (H > 4 || !lanes_kernel(H, combo, MODE_FULL) || (kLanesCombos[combo].rho << kLanesCombos[combo].log_sw) < R) {
-    why = "no lanes-kernel instance for this (n_res, n_hel)";
-    return PWA_OK;
-  }
-  const int rho = kLanesCombos[combo].rho, log_sw = kLanesCombos[combo].log_sw, nw = kLanesCombos[combo].nw;
-  const int prod = kLanesCombos[combo].prod, nthreads = lanes::lanes_threads(nw, prod);
-  const int SW = 1 << log_sw, RP = rho * SW, NW = nw;
-
-  // amplitude rows incl. the zero-filled planes of padding resonances, in nbox boxes of rows_box (<= 256) rows
-  const int rows_need = RP * H;
-  const int nbox = (rows_need + 255) / 256, rows_box = (rows_need + nbox - 1) / nbox;
-  const unsigned amp_bytes = (unsigned)nbox * rows_box * lanes::TILE * 16;
-  const unsigned off_mass = amp_bytes, off_wgt = off_mass + (unsigned)C * lanes::TILE * 8;
-  const unsigned stage_bytes = up(off_wgt + lanes::TILE * 8, 128);
-  const unsigned k_bytes = up((unsigned)RP * lanes::KS * 8, 128);
-  const unsigned red_bytes = up((unsigned)NW * (R * 10 + 2) * 8, 128);
-  const unsigned xch_bytes = up((unsigned)NW * (32 / SW) * 4 * H * 8, 128);
-  const unsigned fixed = k_bytes + red_bytes + xch_bytes + 8u * 2 * 8 + 128;
+  // candidates: every instantiated shape with capacity >= R, smallest capacity first (ties: table order); the first
+  // whose stage fits in shared memory at least twice is taken.  PWA_COMBO forces one entry (A/B runs).
   int dev_smem = 0;
   cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device);
-  int stages = (int)std::min<long long>(8, ((long long)dev_smem - fixed) / stage_bytes);
-  const int st_env = env_int("PWA_STAGES", 0);
-  if (st_env >= 2 && st_env <= stages) stages = st_env;
-  if (stages < 2) { why = "tile does not fit in shared memory"; return PWA_OK; }
+  const int forced = env_int("PWA_COMBO", -1);
+  int combo = -1, stages = 0;
+  int rho = 0, log_sw = 0, nw = 0, prod = 0, tile = 0, SW = 0, RP = 0, NW = 0, nthreads = 0, nbox = 0, rows_box = 0;
+  unsigned amp_bytes = 0, off_mass = 0, off_wgt = 0, stage_bytes = 0, k_bytes = 0, red_bytes = 0, xch_bytes = 0, fixed = 0;
+  why = H > 4 ? "no lanes-kernel instance for this n_hel" : "no lanes-kernel instance for this n_res";
+  std::vector<int> order;
+  for (int k = 0; k < kNumLanesCombos; ++k)
+    if (forced < 0 || k == forced) order.push_back(k);
+  std::stable_sort(order.begin(), order.end(), [](int x, int y) {
+    return (kLanesCombos[x].rho << kLanesCombos[x].log_sw) < (kLanesCombos[y].rho << kLanesCombos[y].log_sw);
+  });
+  {
+    for (size_t oi = 0; oi < order.size() && combo < 0 && H <= 4; ++oi) {
+      const int k = order[oi];
+      const LanesCombo& c = kLanesCombos[k];
+      const int cap = c.rho << c.log_sw;
+      if (cap < R || !lanes_kernel(H, k, MODE_FULL)) continue;
+      rho = c.rho; log_sw = c.log_sw; nw = c.nw; prod = c.prod; tile = c.tile;
+      nthreads = lanes::lanes_threads(nw, prod);
+      SW = 1 << log_sw; RP = rho * SW; NW = nw;
+      if (tile == 32) {
+        // amplitude rows incl. the zero-filled planes of padding resonances, in nbox boxes of rows_box (<= 256) rows
+        const int rows_need = RP * H;
+        nbox = (rows_need + 255) / 256; rows_box = (rows_need + nbox - 1) / nbox;
+        amp_bytes = (unsigned)nbox * rows_box * tile * 16;
+        red_bytes = up((unsigned)NW * (R * 10 + 2) * 8, 128);
+      } else {
+        if (RP > 256) continue;  // one 3-D box [H][RP][8 events]
+        nbox = 1; rows_box = RP;
+        amp_bytes = (unsigned)H * RP * tile * 16;
+        red_bytes = 0;  // the warps add into the block's partial row in turn
+      }
+      off_mass = amp_bytes; off_wgt = up(off_mass + (unsigned)C * tile * 8, 128);  // TMA destinations: 128-byte aligned
+      stage_bytes = up(off_wgt + tile * 8, tile == 32 ? 128 : 1024);
+      k_bytes = up((unsigned)RP * lanes::KS * 8, 128);
+      xch_bytes = up((unsigned)NW * (32 / SW) * 4 * H * 8, 128);
+      fixed = k_bytes + red_bytes + xch_bytes + 8u * 2 * 8 + 128;
+      stages = (int)std::min<long long>(8, ((long long)dev_smem - fixed) / stage_bytes);
+      const int st_env = env_int("PWA_STAGES", 0);
+      if (st_env >= 2 && st_env <= stages) stages = st_env;
+      if (stages < 2) { why = "tile does not fit in shared memory"; continue; }
+      combo = k;
+    }
+  }
+  if (combo < 0) return PWA_OK;
+  why.clear();
   const size_t smem = (size_t)stages * stage_bytes + fixed;
 
   for (int mode = 0; mode < 3; ++mode) {
@@ -118,13 +148,21 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
   for (int sidx = 0; sidx < 2; ++sidx) {
     const SampleDev& d = h->smp[sidx];
     a.n[sidx] = d.n;
-    bool ok = encode_2d(&a.tm_amp[sidx], d.amp, 2ull * d.n, (unsigned long long)R * H, (unsigned long long)d.stride * 16,
-                        2 * lanes::TILE, rows_box, false) &&
-              encode_2d(&a.tm_mass[sidx], d.mass, (unsigned long long)d.n, (unsigned long long)C,
-                        (unsigned long long)d.stride * 8, lanes::TILE, C);
+    bool ok;
+    if (tile == 32) {
+      ok = encode_2d(&a.tm_amp[sidx], d.amp, 2ull * d.n, (unsigned long long)R * H, (unsigned long long)d.stride * 16,
+                     2 * tile, rows_box, false);
+    } else {  // (2 doubles x events, resonance [stride H planes], helicity [stride 1 plane]) -> stage [h][slot][8 events]
+      const unsigned long long dims[3] = {2ull * d.n, (unsigned long long)R, (unsigned long long)H};
+      const unsigned long long strides[2] = {(unsigned long long)H * d.stride * 16, (unsigned long long)d.stride * 16};
+      const unsigned box[3] = {2u * tile, (unsigned)RP, (unsigned)H};
+      ok = encode_3d_swz128(&a.tm_amp[sidx], d.amp, dims, strides, box);
+    }
+    ok = ok && encode_2d(&a.tm_mass[sidx], d.mass, (unsigned long long)d.n, (unsigned long long)C,
+                         (unsigned long long)d.stride * 8, tile, C);
     if (ok && d.weight)
       ok = encode_2d(&a.tm_wgt[sidx], d.weight, (unsigned long long)d.n, 1, up((unsigned)((d.n * 8) & 0x7fffffff), 16) + 16,
-                     lanes::TILE, 1);
+                     tile, 1);
     if (!ok) { why = "cuTensorMapEncodeTiled failed"; return PWA_OK; }
   }
   a.ch = h->d_ch;
@@ -140,7 +178,7 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
   h->variant = 2;
   h->block = nthreads;
   h->grid = h->num_sms;
-  std::snprintf(h->variant_name, sizeof(h->variant_name), "lanes(rho=%d,sw=%d,nw=%d%s,stages=%d)", rho, SW, NW, prod == 2 ? "g" : "", stages);
+  std::snprintf(h->variant_name, sizeof(h->variant_name), "lanes(rho=%d,sw=%d,nw=%d%s,tile=%d,stages=%d)", rho, SW, NW, prod == 2 ? "g" : "", tile, stages);
   return PWA_OK;
 }
 

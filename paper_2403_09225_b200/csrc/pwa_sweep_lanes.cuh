@@ -44,7 +44,7 @@ struct alignas(64) LaneArgs {
 
 namespace lanes {
 
-constexpr int TILE = 32;       // events per tile
+constexpr int TILE32 = 32;     // events per tile (a shape with 6.4 KB per event uses 8-event tiles, see k_sweep_lanes)
 #ifdef PWA_DEBUG_NOLOAD           // timing experiments only: no TMA traffic, compute on whatever the stages hold
 constexpr bool kNoLoad = true;
 #else
@@ -94,6 +94,12 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map
   asm volatile(
       "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(dst),
       "l"(map), "r"(c0), "r"(c1), "r"(bar)
+      : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(dst),
+      "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar)
       : "memory");
 }
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
@@ -220,11 +226,19 @@ __host__ __device__ constexpr int nacc_of() {
 //   2  producer warpgroup: warps 0..3 shrink to 24 registers (setmaxnreg.dec), warp 0 produces; the NW compute warps
 //      4..NW+3 grow to 240 registers (setmaxnreg.inc), so every sub-partition carries NW / 4 compute warps.
 constexpr int lanes_threads(int nw, int prod) { return (nw + (prod == 2 ? 4 : 1)) * 32; }
-template <int H, int RHO, int LOG_SW, int NW, int MODE, int PROD>
+//
+// TILE = 32 (default): amplitude stage = [plane r*H + h][32 events], 512-byte rows, one or two 2-D boxes.
+// TILE = 8 (shapes whose 32-event tile does not fit twice in shared memory, e.g. R = 100, H = 4: 6.4 KB per event):
+//   amplitude stage = [h][resonance slot][8 events] written by ONE 3-D box with the 128-byte swizzle (16-byte chunk
+//   index XOR (row & 7)); the 8 lanes of a quarter-warp own consecutive resonance slots, so their 128-bit reads hit
+//   eight different chunks (conflict-free).  128-byte rows cap the TMA feed near 4.5 TB/s (measured), which such a
+//   shape, bound by the FP64 pipe, does not reach anyway.
+template <int H, int RHO, int LOG_SW, int NW, int MODE, int PROD, int TILE>
 __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(const __grid_constant__ LaneArgs a) {
   constexpr int SW = 1 << LOG_SW;          // slices per warp
   constexpr int EW = 32 / SW;              // events per pass
-  constexpr int NP = SW;                   // passes per tile
+  constexpr int NP = TILE / EW;            // passes per tile
+  static_assert(TILE == 32 || (TILE == 8 && SW >= 8), "8-event tiles need at least 8 slices (swizzle phase = slice & 7)");
   constexpr int NV = (MODE == MODE_FULL ? 4 : 2) * H;  // reals exchanged per event and slice
   constexpr int NACC = nacc_of<MODE>();
   constexpr int NA = NACC > 0 ? NACC : 1;
@@ -272,8 +286,12 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
     const int st = k % stages;
     const uint32_t bar = full0 + 8 * st, dst = smem_u32(smem_raw) + st * a.stage_bytes;
     mbar_expect_tx(bar, a.amp_bytes + (unsigned)a.C * (TILE * 8) + (wg ? TILE * 8u : 0u));
-    for (int x = 0; x < a.nbox; ++x)
-      tma_load_2d(dst + x * a.rows_box * (TILE * 16), &a.tm_amp[smp], 2 * i0, x * a.rows_box, bar);
+    if (TILE == 32) {
+      for (int x = 0; x < a.nbox; ++x)
+        tma_load_2d(dst + x * a.rows_box * (TILE * 16), &a.tm_amp[smp], 2 * i0, x * a.rows_box, bar);
+    } else {
+      tma_load_3d(dst, &a.tm_amp[smp], 2 * i0, 0, 0, bar);
+    }
     tma_load_2d(dst + a.off_mass, &a.tm_mass[smp], i0, 0, bar);
     if (wg) tma_load_2d(dst + a.off_wgt, &a.tm_wgt[smp], i0, 0, bar);
   };
@@ -303,7 +321,7 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
     for (int q = 0; q < NA; ++q) acc[j][q] = 0.0;
   // byte offset of (resonance 0 of this slice, helicity 0, this lane's event in column 0) inside a stage; resonance j,
   // helicity h and the column add compile-time / warp-uniform constants
-  const unsigned lane_f = (unsigned)s * (H * TILE * 16) + (unsigned)e * 16u;
+  const unsigned lane_f = TILE == 32 ? (unsigned)s * (H * TILE * 16) + (unsigned)e * 16u : (unsigned)s * 128u;
   const double* lane_k = Ks + s * KS;
   unsigned moff[RHO];  // byte offset of each own resonance's mass row inside a stage (kept in registers: no dependent load)
 #pragma unroll
@@ -356,7 +374,11 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
       const bool valid = i0 + ev < n;
       if (!kNoLoad) mbar_wait(full0 + 8 * st, (uint32_t)ph);
       const unsigned char* sp = smem_raw + (size_t)st * a.stage_bytes;
-      const unsigned char* fp = sp + lane_f + (col * EW) * 16;
+      // TILE 32: row (j SW + s) H + h, column chunk col EW + e;  TILE 8: row h RP + j SW + s, chunk (col EW + e) ^ (s & 7)
+      const unsigned char* fp = sp + lane_f + (TILE == 32 ? (col * EW) * 16 : (((col * EW + e) ^ (s & 7)) * 16));
+      auto f_at = [&](int j, int h) {
+        return *reinterpret_cast<const double2*>(fp + (TILE == 32 ? (j * SW * H + h) * (TILE * 16) : (h * RP + j * SW) * 128));
+      };
       double wt = 1.0;
       if (weighted) wt = reinterpret_cast<const double*>(sp + a.off_wgt)[ev];
 
@@ -373,7 +395,7 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
           const double zr = fma(c.x, br, -(c.y * bi)), zi = fma(c.x, bi, c.y * br);
 #pragma unroll
           for (int h = 0; h < H; ++h) {
-            const double2 F = *reinterpret_cast<const double2*>(fp + (j * SW * H + h) * (TILE * 16));
+            const double2 F = f_at(j, h);
             if (j == 0) {
               x[2 * h] = fma(zr, F.x, -(zi * F.y));
               x[2 * h + 1] = fma(zr, F.y, zi * F.x);
@@ -391,7 +413,7 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
           }
 #pragma unroll
           for (int h = 0; h < H; ++h) {
-            const double2 F = *reinterpret_cast<const double2*>(fp + (j * SW * H + h) * (TILE * 16));
+            const double2 F = f_at(j, h);
             const double gx = fma(br, F.x, -(bi * F.y)), gy = fma(br, F.y, bi * F.x);
             Gr[j][h] = make_double2(gx, gy);
             if (j == 0) {
@@ -519,40 +541,76 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
     // ---- end of a sample: fixed-order butterfly over the event lanes, fixed-order sum over the warps, one
     //      partial row per block --------------------------------------------------------------------------------
     const int row_len = R * NACC + 2;
-    double* mine = red + (size_t)w * row_len;
-#pragma unroll
-    for (int j = 0; j < RHO; ++j) {
-      const int r = j * SW + s;
-#pragma unroll
-      for (int q = 0; q < NACC; ++q) {
-        double tsum = acc[j][q];
-#pragma unroll
-        for (int m = 1; m < EW; m <<= 1) tsum += shfl_x(tsum, m);
-        if (e == 0 && r < R) mine[r * NACC + q] = tsum;
-        acc[j][q] = 0.0;
-      }
-    }
-    {
-      double t0 = s0, t1 = s1;
-#pragma unroll
-      for (int m = 1; m < EW; m <<= 1) {
-        t0 += shfl_x(t0, m);
-        t1 += shfl_x(t1, m);
-      }
-      if (lane == 0) {  // slice 0, event lane 0
-        mine[R * NACC] = t0;
-        mine[R * NACC + 1] = t1;
-      }
-      s0 = s1 = 0.0;
-    }
-    asm volatile("bar.sync 1, %0;" ::"n"(NW * 32) : "memory");
     double* out = a.partial + ((size_t)smp * gridDim.x + blockIdx.x) * (size_t)row_len;
-    for (int k = w * 32 + lane; k < row_len; k += NW * 32) {
-      double tsum = red[k];
-      for (int ww = 1; ww < NW; ++ww) tsum += red[(size_t)ww * row_len + k];
-      out[k] = tsum;
+    if (TILE == 32) {
+      double* mine = red + (size_t)w * row_len;
+#pragma unroll
+      for (int j = 0; j < RHO; ++j) {
+        const int r = j * SW + s;
+#pragma unroll
+        for (int q = 0; q < NACC; ++q) {
+          double tsum = acc[j][q];
+#pragma unroll
+          for (int m = 1; m < EW; m <<= 1) tsum += shfl_x(tsum, m);
+          if (e == 0 && r < R) mine[r * NACC + q] = tsum;
+          acc[j][q] = 0.0;
+        }
+      }
+      {
+        double t0 = s0, t1 = s1;
+#pragma unroll
+        for (int m = 1; m < EW; m <<= 1) {
+          t0 += shfl_x(t0, m);
+          t1 += shfl_x(t1, m);
+        }
+        if (lane == 0) {  // slice 0, event lane 0
+          mine[R * NACC] = t0;
+          mine[R * NACC + 1] = t1;
+        }
+        s0 = s1 = 0.0;
+      }
+      asm volatile("bar.sync 1, %0;" ::"n"(NW * 32) : "memory");
+      for (int k = w * 32 + lane; k < row_len; k += NW * 32) {
+        double tsum = red[k];
+        for (int ww = 1; ww < NW; ++ww) tsum += red[(size_t)ww * row_len + k];
+        out[k] = tsum;
+      }
+      asm volatile("bar.sync 1, %0;" ::"n"(NW * 32) : "memory");
+    } else {
+      // large shapes keep no per-warp rows in shared memory: the warps add into the block's partial row in turn
+      // (warp 0 writes, warp 1 adds, ...; the same fixed order, one named barrier per turn)
+#pragma unroll 1
+      volatile double* outv = out;  // read back what the previous warp wrote, not a cached copy
+      for (int turn = 0; turn < NW; ++turn) {
+        if (w == turn) {
+#pragma unroll
+          for (int j = 0; j < RHO; ++j) {
+            const int r = j * SW + s;
+#pragma unroll
+            for (int q = 0; q < NACC; ++q) {
+              double tsum = acc[j][q];
+#pragma unroll
+              for (int m = 1; m < EW; m <<= 1) tsum += shfl_x(tsum, m);
+              if (e == 0 && r < R) outv[r * NACC + q] = turn == 0 ? tsum : outv[r * NACC + q] + tsum;
+              acc[j][q] = 0.0;
+            }
+          }
+          double t0 = s0, t1 = s1;
+#pragma unroll
+          for (int m = 1; m < EW; m <<= 1) {
+            t0 += shfl_x(t0, m);
+            t1 += shfl_x(t1, m);
+          }
+          if (lane == 0) {
+            outv[R * NACC] = turn == 0 ? t0 : outv[R * NACC] + t0;
+            outv[R * NACC + 1] = turn == 0 ? t1 : outv[R * NACC + 1] + t1;
+          }
+          s0 = s1 = 0.0;
+          __threadfence_block();
+        }
+        asm volatile("bar.sync 1, %0;" ::"n"(NW * 32) : "memory");
+      }
     }
-    asm volatile("bar.sync 1, %0;" ::"n"(NW * 32) : "memory");
   }
 }
 

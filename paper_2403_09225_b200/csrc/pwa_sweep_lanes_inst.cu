@@ -8,12 +8,12 @@
 
 namespace pwa {
 namespace {
-template <int RHO, int LOG_SW, int NW, int PROD = 0>
+template <int RHO, int LOG_SW, int NW, int PROD = 0, int TILE = 32>
 lanes_fn for_mode(int mode) {
   switch (mode) {
-    case MODE_NLL: return lanes::k_sweep_lanes<PWA_LANES_H, RHO, LOG_SW, NW, MODE_NLL, PROD>;
-    case MODE_GRAD: return lanes::k_sweep_lanes<PWA_LANES_H, RHO, LOG_SW, NW, MODE_GRAD, PROD>;
-    default: return lanes::k_sweep_lanes<PWA_LANES_H, RHO, LOG_SW, NW, MODE_FULL, PROD>;
+    case MODE_NLL: return lanes::k_sweep_lanes<PWA_LANES_H, RHO, LOG_SW, NW, MODE_NLL, PROD, TILE>;
+    case MODE_GRAD: return lanes::k_sweep_lanes<PWA_LANES_H, RHO, LOG_SW, NW, MODE_GRAD, PROD, TILE>;
+    default: return lanes::k_sweep_lanes<PWA_LANES_H, RHO, LOG_SW, NW, MODE_FULL, PROD, TILE>;
   }
 }
 }  // namespace
@@ -32,6 +32,8 @@ lanes_fn PWA_CAT(lanes_kernel_h, PWA_LANES_H)(int combo, int mode) {
     case 7: return for_mode<4, 4, 7>(mode);
     case 8: return for_mode<4, 5, 8, 2>(mode);
     case 9: return for_mode<4, 5, 7>(mode);
+    case 10: return for_mode<4, 4, 8, 2, 8>(mode);
+    case 11: return for_mode<4, 5, 8, 2, 8>(mode);
   }
   return nullptr;
 }

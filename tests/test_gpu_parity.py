@@ -185,3 +185,34 @@ def test_zero_mass_resonance_on_a_ragged_tail(pwa, oracle_mod):
         assert np.isfinite(f) and np.all(np.isfinite(g)) and np.all(np.isfinite(hv))
         assert _nll_err(f, f0) < NLL_TOL and rel_l2(g, g0) < VEC_TOL and rel_l2(hv, h0) < VEC_TOL
         assert pwa.pwa_status_flags(gm.h) == 0
+
+
+@pytest.mark.parametrize("case,combo", [(CASES[2], 10), (CASES[2], 11), (CASES[1], 10), (CASES[0], 11), (CASES[4], 10),
+                                        (CASES[2], 5), (CASES[2], 6), (CASES[1], 3), (CASES[1], 1), (CASES[0], 0)])
+def test_every_kernel_shape_matches_oracle(pwa, oracle_mod, case, combo, monkeypatch):
+    """The handle normally picks one shape per (n_res, n_hel); PWA_COMBO forces another entry of kLanesCombos
+    (csrc/pwa_internal.h) so that every instantiated shape - 8-event swizzled tiles, both producer kinds, every slice
+    count - is compared with the oracle on ragged inputs, not only the ones the default choice reaches."""
+    import workloads
+    cfg, w, om, _ = _case(pwa, oracle_mod, *case)
+    monkeypatch.setenv("PWA_COMBO", str(combo))
+    gm = pwa.Model(w)
+    monkeypatch.delenv("PWA_COMBO")
+    try:
+        name = pwa.pwa_kernel_variant(gm.h)
+        assert name.startswith("lanes"), name
+        if combo >= 10:
+            assert "tile=8" in name, name
+        th = _thetas(cfg)[2]
+        v = workloads.direction(cfg, 9).numpy()
+        f0, g0, h0 = oracle_mod.nll_grad_hvp(om, th, v, "ld")
+        f, g, hv = gm.nll_grad_hvp(th, v)
+        assert _nll_err(f, f0) < NLL_TOL, (name, f, float(f0))
+        assert rel_l2(g, g0) < VEC_TOL and rel_l2(hv, h0) < VEC_TOL, name
+        assert _nll_err(gm.nll(th), f0) < NLL_TOL
+        f1, g1 = gm.nll_grad(th)
+        assert _nll_err(f1, f0) < NLL_TOL and rel_l2(g1, g0) < VEC_TOL
+        f2, g2, hv2 = gm.nll_grad_hvp(th, v)
+        assert g.tobytes() == g2.tobytes() and hv.tobytes() == hv2.tobytes()
+    finally:
+        gm.close()
