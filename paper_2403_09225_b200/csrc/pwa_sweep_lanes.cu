@@ -118,8 +118,8 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
       stage_bytes = up(off_wgt + tile * 8, tile == 32 ? 128 : 1024);
       k_bytes = up((unsigned)RP * lanes::KS * 8, 128);
       xch_bytes = up((unsigned)NW * (32 / SW) * 4 * H * 8, 128);
-      fixed = k_bytes + red_bytes + xch_bytes + 8u * 2 * 8 + 128;
-      stages = (int)std::min<long long>(8, ((long long)dev_smem - fixed) / stage_bytes);
+      fixed = k_bytes + red_bytes + xch_bytes + 32u * 2 * 8 + 128;
+      stages = (int)std::min<long long>(32, ((long long)dev_smem - fixed) / stage_bytes);
       const int st_env = env_int("PWA_STAGES", 0);
       if (st_env >= 2 && st_env <= stages) stages = st_env;
       if (stages < 2) { why = "tile does not fit in shared memory"; continue; }

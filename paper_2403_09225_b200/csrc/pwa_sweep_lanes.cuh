@@ -231,8 +231,9 @@ constexpr int lanes_threads(int nw, int prod) { return (nw + (prod == 2 ? 4 : 1)
 // TILE = 8 (shapes whose 32-event tile does not fit twice in shared memory, e.g. R = 100, H = 4: 6.4 KB per event):
 //   amplitude stage = [h][resonance slot][8 events] written by ONE 3-D box with the 128-byte swizzle (16-byte chunk
 //   index XOR (row & 7)); the 8 lanes of a quarter-warp own consecutive resonance slots, so their 128-bit reads hit
-//   eight different chunks (conflict-free).  128-byte rows cap the TMA feed near 4.5 TB/s (measured), which such a
-//   shape, bound by the FP64 pipe, does not reach anyway.
+//   eight different chunks (conflict-free).  128-byte rows cap the TMA feed near 4.1 TB/s whatever the ring depth
+//   (measured with this layout on config 3 in NLL mode: 0.62 of the HBM peak against 1.05 for 512-byte rows), so
+//   this variant is only chosen when the 32-event tile does not fit; config 4 runs at that cap.
 template <int H, int RHO, int LOG_SW, int NW, int MODE, int PROD, int TILE>
 __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(const __grid_constant__ LaneArgs a) {
   constexpr int SW = 1 << LOG_SW;          // slices per warp
