@@ -90,15 +90,26 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+_ORACLE_MODELS = {}
+
+
 def _oracle_sample_time(w, n_mc_s, n_data_s, th, v, threads):
-    """Times the CPU oracle (double build, OpenMP) on the first n_mc_s / n_data_s events of the workload."""
+    """Times the CPU oracle (double build, OpenMP) on the first n_mc_s / n_data_s events of the workload
+    (the host copy of the sample is made once and is not part of the timed region)."""
     import oracle
     import numpy as np
+    key = (id(w), n_mc_s, n_data_s)
+    if key in _ORACLE_MODELS:
+        m = _ORACLE_MODELS[key]
+        t0 = time.perf_counter()
+        out = oracle.nll_grad_hvp(m, np.asarray(th), np.asarray(v), "d", threads=threads)
+        return time.perf_counter() - t0, out
     to_np = lambda t: None if t is None else t.detach().cpu().numpy()
     data = oracle.Sample(to_np(w.data_mass[:, :n_data_s]), to_np(w.data_amp[:, :, :n_data_s]),
                          to_np(None if w.data_weight is None else w.data_weight[:n_data_s]))
     mc = oracle.Sample(to_np(w.mc_mass[:, :n_mc_s]), to_np(w.mc_amp[:, :, :n_mc_s]), None)
     m = oracle.Model(to_np(w.res_chan), data, mc)
+    _ORACLE_MODELS[key] = m
     t0 = time.perf_counter()
     out = oracle.nll_grad_hvp(m, np.asarray(th), np.asarray(v), "d", threads=threads)
     return time.perf_counter() - t0, out
@@ -368,10 +379,18 @@ def main():
         threads = oracle.max_threads()
         n_mc_s = min(cfg.n_mc, args.ref_events)
         n_data_s = max(1, n_mc_s * cfg.n_data // cfg.n_mc)
-        dt, out = _oracle_sample_time(w, n_mc_s, n_data_s, th_np, v_np, threads)
-        line["cpu_baseline"] = {"value": (n_mc_s + n_data_s) / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
-                                "sample": f"first {n_mc_s} MC + {n_data_s} data events of the same arrays, one "
-                                          f"NLL+grad+HVP evaluation ({dt:.1f} s)"}
+        # repeat the evaluation until about 10 s of CPU work have been timed (bounded: at most 40 evaluations)
+        total, reps = 0.0, 0
+        while reps < 40 and (total < 10.0 or reps < 2):
+            dt, out = _oracle_sample_time(w, n_mc_s, n_data_s, th_np, v_np, threads)
+            total += dt
+            reps += 1
+        line["cpu_baseline"] = {"value": reps * (n_mc_s + n_data_s) / total, "unit": UNIT, "cores": threads,
+                                "kind": "oracle",
+                                "sample": f"first {n_mc_s} MC + {n_data_s} data events of the same arrays, {reps} "
+                                          f"NLL+grad+HVP evaluations ({total:.1f} s)",
+                                "nll_rel_diff_vs_gpu": abs(float(out[0]) - nll_dev) / max(abs(float(out[0])), 1.0)
+                                if (n_mc_s == cfg.n_mc and world == 1) else None}
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
