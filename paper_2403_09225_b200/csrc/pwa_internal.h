@@ -66,7 +66,7 @@ struct LanesCombo {
 };
 // instantiated shapes (pwa_sweep_lanes_inst.cu); capacity RHO << LOG_SW resonances; the handle takes the first entry of
 // the smallest capacity >= R whose stages fit in shared memory at least twice
-constexpr LanesCombo kLanesCombos[] = {{1, 2, 15, 0, 32}, {2, 3, 15, 0, 32}, {3, 2, 8, 2, 32}, {3, 2, 11, 0, 32}, {4, 3, 8, 2, 32},
+constexpr LanesCombo kLanesCombos[] = {{1, 2, 15, 0, 32}, {2, 3, 15, 0, 32}, {3, 2, 11, 0, 32}, {3, 2, 8, 2, 32}, {4, 3, 8, 2, 32},
                                        {4, 3, 7, 0, 32}, {4, 4, 8, 2, 32}, {4, 4, 7, 0, 32}, {4, 5, 8, 2, 32}, {4, 5, 7, 0, 32},
                                        {4, 4, 8, 2, 8}, {4, 5, 8, 2, 8}};
 constexpr int kNumLanesCombos = sizeof(kLanesCombos) / sizeof(kLanesCombos[0]);

@@ -119,9 +119,10 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
       k_bytes = up((unsigned)RP * lanes::KS * 8, 128);
       xch_bytes = up((unsigned)NW * (32 / SW) * 4 * H * 8, 128);
       fixed = k_bytes + red_bytes + xch_bytes + 32u * 2 * 8 + 128;
-      stages = (int)std::min<long long>(32, ((long long)dev_smem - fixed) / stage_bytes);
+      const int fit = (int)std::min<long long>(32, ((long long)dev_smem - fixed) / stage_bytes);
+      stages = std::min(8, fit);  // deeper rings were measured no faster (the kernel is not feed-bound); PWA_STAGES overrides
       const int st_env = env_int("PWA_STAGES", 0);
-      if (st_env >= 2 && st_env <= stages) stages = st_env;
+      if (st_env >= 2 && st_env <= fit) stages = st_env;
       if (stages < 2) { why = "tile does not fit in shared memory"; continue; }
       combo = k;
     }

@@ -24,8 +24,8 @@ lanes_fn PWA_CAT(lanes_kernel_h, PWA_LANES_H)(int combo, int mode) {
   switch (combo) {
     case 0: return for_mode<1, 2, 15>(mode);
     case 1: return for_mode<2, 3, 15>(mode);
-    case 2: return for_mode<3, 2, 8, 2>(mode);
-    case 3: return for_mode<3, 2, 11>(mode);
+    case 2: return for_mode<3, 2, 11>(mode);
+    case 3: return for_mode<3, 2, 8, 2>(mode);
     case 4: return for_mode<4, 3, 8, 2>(mode);
     case 5: return for_mode<4, 3, 7>(mode);
     case 6: return for_mode<4, 4, 8, 2>(mode);
