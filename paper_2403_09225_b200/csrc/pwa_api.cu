@@ -59,6 +59,9 @@ static sweep_fn generic_fn(int H, int mode) {
   }
 }
 
+// blocks of the second reduction stage (phase 1 is spread over them, the last one to finish does the rest)
+static constexpr int kReduceBlocks = 8;
+
 static inline int nb_of(int R, int mode) {
   if (mode == MODE_NLL) return 0;
   const int rpb = rpb_of(mode);
@@ -68,7 +71,8 @@ static inline int nb_of(int R, int mode) {
 static size_t generic_smem(int block, int nb) { return (size_t)(block / 32) * ((size_t)nb * 32 + 2) * sizeof(double); }
 
 // Runs prologue + sweep + stage-2 reduction/unpack; leaves the public raw vector in `raw` (device).
-static pwa_status raw_sums_impl(pwa_handle* h, int mode, const double* theta, const double* v, double* raw) {
+static pwa_status raw_sums_impl(pwa_handle* h, int mode, const double* theta, const double* v, double* raw,
+                                bool combine = false, double* nll = nullptr, double* grad = nullptr, double* hv = nullptr) {
   const int R = h->n_res;
   if (mode == MODE_FULL && !v) mode = MODE_GRAD;
   const bool prof = h->profiling && h->prof_used + 2 <= h->prof_events.size();
@@ -110,13 +114,16 @@ static pwa_status raw_sums_impl(pwa_handle* h, int mode, const double* theta, co
   const double n_mc = (double)h->smp[0].n;
   switch (mode) {
     case MODE_NLL:
-      k_reduce_unpack<MODE_NLL><<<1, 1024, 0, h->stream>>>(h->d_partial, h->grid, nb, R, packed, theta, v, n_mc, h->d_sums, raw);
+      k_reduce_unpack<MODE_NLL><<<kReduceBlocks, 1024, 0, h->stream>>>(h->d_partial, h->grid, nb, R, packed, theta, v, n_mc, h->d_sums, raw,
+                                                             combine ? 1 : 0, nll, grad, hv, h->d_flags, h->d_flags + 1);
       break;
     case MODE_GRAD:
-      k_reduce_unpack<MODE_GRAD><<<1, 1024, 0, h->stream>>>(h->d_partial, h->grid, nb, R, packed, theta, v, n_mc, h->d_sums, raw);
+      k_reduce_unpack<MODE_GRAD><<<kReduceBlocks, 1024, 0, h->stream>>>(h->d_partial, h->grid, nb, R, packed, theta, v, n_mc, h->d_sums, raw,
+                                                             combine ? 1 : 0, nll, grad, hv, h->d_flags, h->d_flags + 1);
       break;
     default:
-      k_reduce_unpack<MODE_FULL><<<1, 1024, 0, h->stream>>>(h->d_partial, h->grid, nb, R, packed, theta, v, n_mc, h->d_sums, raw);
+      k_reduce_unpack<MODE_FULL><<<kReduceBlocks, 1024, 0, h->stream>>>(h->d_partial, h->grid, nb, R, packed, theta, v, n_mc, h->d_sums, raw,
+                                                             combine ? 1 : 0, nll, grad, hv, h->d_flags, h->d_flags + 1);
       break;
   }
   h->launches++;
@@ -133,9 +140,8 @@ static pwa_status combine_impl(pwa_handle* h, const double* raw, const double* v
 }
 
 pwa_status eval(pwa_handle* h, int mode, const double* theta, const double* v, double* nll, double* grad, double* hv) {
-  pwa_status st = raw_sums_impl(h, mode, theta, v, h->d_raw);
-  if (st != PWA_OK) return st;
-  return combine_impl(h, h->d_raw, (mode == MODE_FULL) ? v : nullptr, nll, grad, (mode == MODE_FULL) ? hv : nullptr);
+  // sweep, then ONE launch for the second reduction stage, the unpacking and Eqs. 4, 6, 7
+  return raw_sums_impl(h, mode, theta, v, h->d_raw, true, nll, grad, hv);
 }
 
 }  // namespace pwa
@@ -291,7 +297,7 @@ extern "C" pwa_status pwa_create(const pwa_model_desc* m, pwa_handle** out) {
             cudaMalloc(&h->d_partial, sizeof(double) * h->partial_doubles) == cudaSuccess &&
             cudaMalloc(&h->d_sums, sizeof(double) * 2 * pstride) == cudaSuccess &&
             cudaMalloc(&h->d_raw, sizeof(double) * (4 + 4 * (size_t)P)) == cudaSuccess &&
-            cudaMalloc(&h->d_flags, sizeof(unsigned)) == cudaSuccess &&
+            cudaMalloc(&h->d_flags, 2 * sizeof(unsigned)) == cudaSuccess &&
             cudaMalloc(&h->d_io, sizeof(double) * io) == cudaSuccess &&
             cudaMalloc(&h->d_fit, sizeof(double) * (8 * (size_t)P + 64)) == cudaSuccess &&
             cudaMallocHost(&h->h_pin, sizeof(double) * io) == cudaSuccess &&
@@ -301,7 +307,7 @@ extern "C" pwa_status pwa_create(const pwa_model_desc* m, pwa_handle** out) {
     return fail_create(h, PWA_ERR_OOM, "scratch allocation failed");
   }
   if ((ce = cudaMemcpyAsync(h->d_ch, m->res_chan, sizeof(int) * R, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
-      (ce = cudaMemsetAsync(h->d_flags, 0, sizeof(unsigned), h->stream)) != cudaSuccess ||
+      (ce = cudaMemsetAsync(h->d_flags, 0, 2 * sizeof(unsigned), h->stream)) != cudaSuccess ||
       (ce = cudaStreamSynchronize(h->stream)) != cudaSuccess)
     return fail_create(h, PWA_ERR_CUDA, std::string("upload: ") + cudaGetErrorString(ce));
   *out = h;

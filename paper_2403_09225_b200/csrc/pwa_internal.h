@@ -26,7 +26,7 @@ struct pwa_handle {
   double* d_partial = nullptr;  // per-block partial sums
   double* d_sums = nullptr;     // block-summed compact sums
   double* d_raw = nullptr;      // public raw vector (4 + 4P)
-  unsigned* d_flags = nullptr;
+  unsigned* d_flags = nullptr;  // [0] non-finite flag of the last evaluation, [1] ticket counter of the reduction kernel
   size_t partial_doubles = 0;
 
   // sweep launch configuration (fixed at creation -> deterministic event -> thread map)

@@ -287,68 +287,14 @@ __device__ inline void unpack_res(const Sums5& s, double a, double phi, double M
   h4[3] = 2.0 * t.re;
 }
 
-// packed = 1: partial rows are [R][VPR] + 2 scalars (tiled TMA sweep); packed = 0: [nb][32] + 2 (generic sweep)
-template <int MODE>
-__global__ void __launch_bounds__(1024) k_reduce_unpack(const double* __restrict__ partial, int nblocks, int nb, int R,
-                                                        int packed, const double* __restrict__ theta,
-                                                        const double* __restrict__ v, double n_mc,
-                                                        double* __restrict__ sums, double* __restrict__ raw) {
-  constexpr int VPR = vpr_of(MODE), RPB = rpb_of(MODE);
-  const int nacc = packed ? (MODE == MODE_NLL ? 0 : R * VPR) : nb * 32, stride = nacc + 2, P = 4 * R;
-  for (int k = threadIdx.x; k < 2 * stride; k += blockDim.x) {
-    const int sample = k / stride, idx = k - sample * stride;
-    const double* p = partial + (size_t)sample * nblocks * stride + idx;
-    double t = 0.0;
-    for (int b = 0; b < nblocks; ++b) t += p[(size_t)b * stride];
-    sums[k] = t;
-  }
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    raw[0] = sums[stride + nacc];      // sum_data w ln I
-    raw[1] = sums[stride + nacc + 1];  // W
-    raw[2] = sums[nacc];               // G
-    raw[3] = n_mc;
-  }
-  if (MODE == MODE_NLL) {
-    for (int k = threadIdx.x; k < 4 * P; k += blockDim.x) raw[4 + k] = 0.0;
-    return;
-  }
-  for (int r = threadIdx.x; r < R; r += blockDim.x) {
-    const int b = r / RPB, j = r - b * RPB;
-    const int qoff = packed ? r * VPR : b * 32 + j * VPR;
-    const double a = theta[4 * r], phi = theta[4 * r + 1], M = theta[4 * r + 2], G = theta[4 * r + 3];
-    for (int sample = 0; sample < 2; ++sample) {
-      const double* q = sums + (size_t)sample * stride + qoff;
-      Sums5 s;
-      s.P1 = {q[0], q[1]};
-      s.P2 = {q[2], q[3]};
-      if (MODE == MODE_FULL) {
-        s.P3 = {q[4], q[5]};
-        s.Q1 = {q[6], q[7]};
-        s.Q2 = {q[8], q[9]};
-      } else {
-        s.P3 = s.Q1 = s.Q2 = {0.0, 0.0};
-      }
-      double g4[4], h4[4] = {0.0, 0.0, 0.0, 0.0};
-      unpack_res(s, a, phi, M, G, (MODE == MODE_FULL && v) ? v + 4 * r : nullptr, g4, h4);
-      // raw layout: gd | gG | hd | hG ; data (sample 1) carries hd = -h
-      double* gdst = raw + 4 + (sample == 1 ? 0 : P) + 4 * r;
-      double* hdst = raw + 4 + 2 * P + (sample == 1 ? 0 : P) + 4 * r;
-      for (int k = 0; k < 4; ++k) {
-        gdst[k] = g4[k];
-        hdst[k] = sample == 1 ? -h4[k] : h4[k];
-      }
-    }
-  }
-}
-
 // ------------------------------------------------------------------------------------------------
 // Combine: Eqs. 4, 6, 7 with NLL = -lnL and N_Data := W (S2, S3, S9).
-// One block; any of nll / grad / hv may be null.  Sets bit0 of *flags when a result is not finite.
+// One block of 1024 threads; any of nll / grad / hv may be null.  Sets bit0 of *flags when a result is not finite.
+// raw may have been written by this very block (fused path): plain loads, no read-only cache.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(1024) k_combine(const double* __restrict__ raw, const double* __restrict__ v, int P,
-                                                  double* __restrict__ nll, double* __restrict__ grad,
-                                                  double* __restrict__ hv, unsigned* __restrict__ flags) {
+__device__ __forceinline__ void combine_block(const double* raw, const double* __restrict__ v, int P, double* __restrict__ nll,
+                                              double* __restrict__ grad, double* __restrict__ hv,
+                                              unsigned* __restrict__ flags) {
   __shared__ double red[1024];
   __shared__ int bad;
   const double Ld = raw[0], W = raw[1], G = raw[2], n_mc = raw[3];
@@ -394,6 +340,104 @@ __global__ void __launch_bounds__(1024) k_combine(const double* __restrict__ raw
   if (mybad) atomicOr(&bad, 1);
   __syncthreads();
   if (threadIdx.x == 0) *flags = bad ? 1u : 0u;
+}
+
+__global__ void __launch_bounds__(1024) k_combine(const double* raw, const double* __restrict__ v, int P,
+                                                  double* __restrict__ nll, double* __restrict__ grad,
+                                                  double* __restrict__ hv, unsigned* __restrict__ flags) {
+  combine_block(raw, v, P, nll, grad, hv, flags);
+}
+
+// Second reduction stage (a-7): fixed-order sum of the per-block partial rows, compact sums -> raw sums
+// (SURVEY appendix), and - when `combine` is set - Eqs. 4, 6, 7 in the same launch (the evaluation calls; the
+// shard interface pwa_raw_sums stops at the raw vector).
+// packed = 1: partial rows are [R][VPR] + 2 scalars (lanes sweep); packed = 0: [nb][32] + 2 (generic sweep)
+template <int MODE>
+__global__ void __launch_bounds__(1024) k_reduce_unpack(const double* __restrict__ partial, int nblocks, int nb, int R,
+                                                        int packed, const double* __restrict__ theta,
+                                                        const double* __restrict__ v, double n_mc, double* sums, double* raw,
+                                                        int combine, double* __restrict__ nll, double* __restrict__ grad,
+                                                        double* __restrict__ hv, unsigned* __restrict__ flags,
+                                                        unsigned* ticket) {
+  constexpr int VPR = vpr_of(MODE), RPB = rpb_of(MODE);
+  const int nacc = packed ? (MODE == MODE_NLL ? 0 : R * VPR) : nb * 32, stride = nacc + 2, P = 4 * R;
+  // Phase 1 over all blocks of this launch: block g sums the columns k = g * 1024 + t, (g + gridDim) * 1024 + t, ...
+  // (one SM cannot pull the 148 partial rows fast enough on its own).  The value of every column is independent of
+  // the block that computes it.
+  for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < 2 * stride; k += gridDim.x * blockDim.x) {
+    const int sample = k / stride, idx = k - sample * stride;
+    const double* p = partial + (size_t)sample * nblocks * stride + idx;
+    // four interleaved running sums (rows b = 0, 4, 8, ... / 1, 5, ... / ...) keep four loads in flight; the order of
+    // additions is fixed: ((t0 + t1) + (t2 + t3))
+    double t0 = 0.0, t1 = 0.0, t2 = 0.0, t3 = 0.0;
+    int b = 0;
+#pragma unroll 2
+    for (; b + 4 <= nblocks; b += 4) {
+      t0 += p[(size_t)b * stride];
+      t1 += p[(size_t)(b + 1) * stride];
+      t2 += p[(size_t)(b + 2) * stride];
+      t3 += p[(size_t)(b + 3) * stride];
+    }
+    for (; b < nblocks; ++b) t0 += p[(size_t)b * stride];
+    sums[k] = (t0 + t1) + (t2 + t3);
+  }
+  // The block that finishes last (whichever it is: the sums do not depend on it) unpacks and combines.
+  if (gridDim.x > 1) {
+    __shared__ unsigned last;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      const unsigned done = atomicAdd(ticket, 1u);
+      last = done == gridDim.x - 1 ? 1u : 0u;
+      if (last) *ticket = 0u;  // ready for the next launch on this stream
+    }
+    __syncthreads();
+    if (!last) return;
+    __threadfence();  // what the other blocks wrote is read below with L2-only loads (__ldcg)
+  } else {
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    raw[0] = __ldcg(sums + stride + nacc);      // sum_data w ln I
+    raw[1] = __ldcg(sums + stride + nacc + 1);  // W
+    raw[2] = __ldcg(sums + nacc);               // G
+    raw[3] = n_mc;
+  }
+  if (MODE == MODE_NLL) {
+    for (int k = threadIdx.x; k < 4 * P; k += blockDim.x) raw[4 + k] = 0.0;
+  } else {
+    for (int r = threadIdx.x; r < R; r += blockDim.x) {
+      const int b = r / RPB, j = r - b * RPB;
+      const int qoff = packed ? r * VPR : b * 32 + j * VPR;
+      const double a = theta[4 * r], phi = theta[4 * r + 1], M = theta[4 * r + 2], G = theta[4 * r + 3];
+      for (int sample = 0; sample < 2; ++sample) {
+        const double* q = sums + (size_t)sample * stride + qoff;
+        Sums5 s;
+        s.P1 = {__ldcg(q), __ldcg(q + 1)};
+        s.P2 = {__ldcg(q + 2), __ldcg(q + 3)};
+        if (MODE == MODE_FULL) {
+          s.P3 = {__ldcg(q + 4), __ldcg(q + 5)};
+          s.Q1 = {__ldcg(q + 6), __ldcg(q + 7)};
+          s.Q2 = {__ldcg(q + 8), __ldcg(q + 9)};
+        } else {
+          s.P3 = s.Q1 = s.Q2 = {0.0, 0.0};
+        }
+        double g4[4], h4[4] = {0.0, 0.0, 0.0, 0.0};
+        unpack_res(s, a, phi, M, G, (MODE == MODE_FULL && v) ? v + 4 * r : nullptr, g4, h4);
+        // raw layout: gd | gG | hd | hG ; data (sample 1) carries hd = -h
+        double* gdst = raw + 4 + (sample == 1 ? 0 : P) + 4 * r;
+        double* hdst = raw + 4 + 2 * P + (sample == 1 ? 0 : P) + 4 * r;
+        for (int k = 0; k < 4; ++k) {
+          gdst[k] = g4[k];
+          hdst[k] = sample == 1 ? -h4[k] : h4[k];
+        }
+      }
+    }
+  }
+  if (combine) {
+    __syncthreads();  // the raw vector of this block's own writes is visible to the whole block
+    combine_block(raw, (MODE == MODE_FULL) ? v : nullptr, P, nll, grad, (MODE == MODE_FULL) ? hv : nullptr, flags);
+  }
 }
 
 }  // namespace pwa
