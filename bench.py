@@ -391,6 +391,11 @@ def main():
                                           f"NLL+grad+HVP evaluations ({total:.1f} s)",
                                 "nll_rel_diff_vs_gpu": abs(float(out[0]) - nll_dev) / max(abs(float(out[0])), 1.0)
                                 if (n_mc_s == cfg.n_mc and world == 1) else None}
+        # the same oracle on ONE thread, on a tenth of the sample ("plus a 1-thread figure")
+        n1_mc, n1_d = max(1, n_mc_s // 10), max(1, n_data_s // 10)
+        dt1, _ = _oracle_sample_time(w, n1_mc, n1_d, th_np, v_np, 1)
+        line["cpu_baseline"]["one_thread"] = {"value": (n1_mc + n1_d) / dt1, "unit": UNIT,
+                                              "sample": f"first {n1_mc} MC + {n1_d} data events, one evaluation ({dt1:.1f} s)"}
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()

@@ -216,3 +216,39 @@ def test_every_kernel_shape_matches_oracle(pwa, oracle_mod, case, combo, monkeyp
         assert g.tobytes() == g2.tobytes() and hv.tobytes() == hv2.tobytes()
     finally:
         gm.close()
+
+
+def test_many_repeats_bit_identical_under_load(pwa, oracle_mod):
+    """A race in the TMA ring, the shared-memory exchange rows or the ticketed reduction would show up as a changed
+    bit in some repeat (compute-sanitizer is not available on the GPU pool).  150 back-to-back evaluations in all
+    three kernel modes on a config-3-shaped sample large enough to wrap the ring many times."""
+    import workloads
+    cfg = workloads.CONFIGS[3].scaled(300_007, 30_011)
+    w = workloads.make_workload(cfg, torch.device("cuda", 0))
+    gm = pwa.Model(w, borrow=True)
+    try:
+        dev = torch.device("cuda", 0)
+        th = torch.tensor(workloads.random_start(cfg, 1).numpy(), device=dev)
+        v = torch.tensor(workloads.direction(cfg, 2).numpy(), device=dev)
+        P = cfg.n_par
+        outs = torch.zeros(150, 2 + 3 * P, dtype=torch.float64, device=dev)
+        for k in range(150):
+            row = outs[k]
+            pwa.pwa_nll_grad_hvp(gm.h, th, v, row[0:1], row[2:2 + P], row[2 + P:2 + 2 * P])
+            if k % 3 == 0:
+                pwa.pwa_nll(gm.h, th, row[1:2])
+            else:
+                pwa.pwa_nll_grad(gm.h, th, row[1:2], row[2 + 2 * P:2 + 3 * P])
+        torch.cuda.synchronize()
+        o = outs.cpu().numpy()
+        assert np.all(np.isfinite(o))
+        for k in range(1, 150):
+            assert o[k, 0].tobytes() == o[0, 0].tobytes() and o[k, 2:2 + 2 * P].tobytes() == o[0, 2:2 + 2 * P].tobytes(), k
+            assert o[k, 1].tobytes() == o[0, 1].tobytes() or k % 3 != 0
+        # the three modes agree on the NLL to rounding (different instruction mixes, same sums)
+        assert abs(o[0, 1] - o[0, 0]) <= 1e-12 * abs(o[0, 0]) and abs(o[1, 1] - o[0, 0]) <= 1e-12 * abs(o[0, 0])
+        gr = [k for k in range(150) if k % 3 != 0]
+        for k in gr[1:]:
+            assert o[k, 2 + 2 * P:].tobytes() == o[gr[0], 2 + 2 * P:].tobytes(), k
+    finally:
+        gm.close()
