@@ -373,6 +373,15 @@ def main():
         "gpu_launches": int(launches),
         "clocks": clocks,
     }
+    # the ALU co-limit beside the HBM roofline: FP64 instructions the method needs per event
+    # (16 R H + 52 R + 80 DFMA-class) against the FP64 pipe rate measured on this pool
+    # (profiles/r01_microbench.md: 17.05 T DFMA/s sustained)
+    fp64_per_event = 16 * cfg.n_res * cfg.n_hel + 52 * cfg.n_res + 80
+    if sweep_n:
+        rate = fp64_per_event * events_per_step / sweep_avg_s / 1e12
+        line["fp64_pipe"] = {"dfma_class_per_event": fp64_per_event, "achieved": rate, "peak": 17.05,
+                             "unit": "T instr/s", "frac": rate / 17.05,
+                             "peak_source": "measured (profiles/r01_microbench.md, fp64_peak)"}
     if not args.no_cpu_baseline:
         import oracle
         oracle.build()

@@ -91,3 +91,13 @@ def test_nonfinite_start_is_reported(setup):
     assert res.status == 4  # PWA_ERR_NONFINITE, reported in the result, theta left at the start point
     assert np.array_equal(th, th0)
     assert pwa.pwa_status_flags(gm.h) & 1
+
+
+def test_wall_time_cap_stops_the_fit(setup):
+    """PAPER.md:135 ("early stopping"): max_seconds ends the fit at the next outer iteration with stop_reason 5."""
+    pwa, workloads, models = setup
+    cfg, w, om, gm = models[2]
+    th0 = workloads.random_start(cfg, 0).numpy()
+    th, res = gm.fit(th0, _opts(pwa, max_seconds=1e-7))
+    assert res.stop_reason == 5 and res.status == 5 and res.outer_iters <= 1
+    assert np.isfinite(res.nll) and res.nll <= gm.nll(th0) + 1e-9 * abs(res.nll)
