@@ -154,6 +154,12 @@ pwa_status pwa_fit_newton_cg(pwa_handle* h, double* theta_inout, const pwa_fit_o
 pwa_status pwa_nll_grad_hvp_host(pwa_handle* h, const double* theta_host, const double* v_host,
                                  double* nll_host, double* grad_host, double* hv_host);
 
+/* ---- fit fractions (Table 1 of the paper lists a "fraction" F_i per resonance; S20) ----
+ * frac[r] = sum_mc sum_h |c_r B_r(j) F_rh(j)|^2 / sum_mc I_j  over the handle's phase-space MC sample.
+ * theta: DEVICE pointer, P doubles; frac: DEVICE pointer, n_res doubles.  Enqueues on the handle's stream (one pass
+ * over the MC event store), does not synchronise.  PWA_ERR_INVALID_ARG on null pointers. */
+pwa_status pwa_fit_fractions(pwa_handle* h, const double* theta, double* frac);
+
 /* ---- diagnostics -------------------------------------------------------------------------------*/
 /* Synchronises; *flags_host bit0 = the last evaluation produced a non-finite NLL, gradient or HVP. */
 pwa_status pwa_status_flags(pwa_handle* h, uint32_t* flags_host);

@@ -252,3 +252,16 @@ def test_many_repeats_bit_identical_under_load(pwa, oracle_mod):
             assert o[k, 2 + 2 * P:].tobytes() == o[gr[0], 2 + 2 * P:].tobytes(), k
     finally:
         gm.close()
+
+
+@pytest.mark.parametrize("idx,n_mc,n_data", CASES)
+def test_fit_fractions_match_oracle(pwa, oracle_mod, idx, n_mc, n_data):
+    """pwa_fit_fractions (S20) against oracle/fractions.py, element by element, 1e-10 relative."""
+    from oracle.fractions import fit_fractions
+    cfg, w, om, gm = _case(pwa, oracle_mod, idx, n_mc, n_data)
+    for th in _thetas(cfg)[:2]:
+        f0 = fit_fractions(om, th)
+        f = gm.fit_fractions(th)
+        assert f.shape == f0.shape and np.all(np.isfinite(f))
+        assert np.max(np.abs(f - f0) / f0) < 1e-10, idx
+        assert gm.fit_fractions(th).tobytes() == f.tobytes()  # repeat runs bit-identical
