@@ -95,6 +95,16 @@ pwa_status pwa_hvp(pwa_handle* h, const double* theta, const double* v, double* 
 pwa_status pwa_nll_grad_hvp(pwa_handle* h, const double* theta, const double* v, double* nll,
                             double* grad, double* hv);
 
+/* ---- split evaluation for Newton-CG (the optimiser asks for many HVPs at one theta) -------------
+ * pwa_nll_grad_for_hvp = pwa_nll_grad that also keeps, inside the handle, a copy of theta and the direction-
+ * independent sums of the HVP (the compact sums P1, P2, P3 of DESIGN.md section 5.1).  pwa_hvp_cached(v) then gives
+ * H(theta) v for the theta of the LAST pwa_nll_grad_for_hvp call with a lighter sweep (only the v-dependent sums:
+ * 49 instead of 69 FP64 instructions per event and resonance).  Results equal pwa_hvp(theta, v) to rounding.
+ * Other calls (pwa_nll, pwa_nll_grad, pwa_hvp, pwa_raw_sums ...) may come in between: they do not touch what is kept.
+ * pwa_hvp_cached before any pwa_nll_grad_for_hvp: PWA_ERR_INVALID_ARG.  Device pointers, enqueue only. */
+pwa_status pwa_nll_grad_for_hvp(pwa_handle* h, const double* theta, double* nll, double* grad);
+pwa_status pwa_hvp_cached(pwa_handle* h, const double* v, double* hv);
+
 /* ---- shard interface (Eqs. 4-7) -----------------------------------------------
  * pwa_raw_sums runs the same streaming pass but stops before the logarithm / division of Eqs. 4, 6, 7
  * and writes the ADDITIVE raw sums of this handle's events:  raw[pwa_raw_size(h)] doubles (device)

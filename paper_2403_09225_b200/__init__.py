@@ -17,6 +17,7 @@ from typing import Optional
 __all__ = ["PwaError", "lib_path", "load", "pwa_create", "pwa_destroy", "pwa_n_params", "pwa_raw_size", "pwa_nll",
            "pwa_nll_grad", "pwa_hvp", "pwa_nll_grad_hvp", "pwa_raw_sums", "pwa_combine", "pwa_fit_opts",
            "pwa_fit_result", "pwa_fit_opts_default", "pwa_fit_newton_cg", "pwa_nll_grad_hvp_host", "pwa_fit_fractions",
+           "pwa_nll_grad_for_hvp", "pwa_hvp_cached",
            "pwa_status_flags", "pwa_profile_enable", "pwa_profile_read", "pwa_kernel_launches", "pwa_bytes_per_eval",
            "pwa_kernel_variant", "pwa_last_error", "pwa_version", "Model", "STATUS_NAMES", "EXPORTS"]
 
@@ -31,7 +32,7 @@ PWA_MEM_HOST, PWA_MEM_DEVICE = 0, 1
 # every symbol include/pwa.h declares
 EXPORTS = ["pwa_create", "pwa_destroy", "pwa_n_params", "pwa_nll", "pwa_nll_grad", "pwa_hvp", "pwa_nll_grad_hvp",
            "pwa_raw_size", "pwa_raw_sums", "pwa_combine", "pwa_fit_opts_default", "pwa_fit_newton_cg",
-           "pwa_nll_grad_hvp_host", "pwa_fit_fractions", "pwa_status_flags", "pwa_profile_enable", "pwa_profile_read",
+           "pwa_nll_grad_hvp_host", "pwa_fit_fractions", "pwa_nll_grad_for_hvp", "pwa_hvp_cached", "pwa_status_flags", "pwa_profile_enable", "pwa_profile_read",
            "pwa_kernel_launches", "pwa_bytes_per_eval", "pwa_kernel_variant", "pwa_last_error", "pwa_version"]
 
 
@@ -98,6 +99,8 @@ def load():
     lib.pwa_fit_newton_cg.argtypes = [vp, dp, POINTER(pwa_fit_opts), POINTER(pwa_fit_result)]
     lib.pwa_nll_grad_hvp_host.argtypes = [vp, dp, dp, dp, dp, dp]
     lib.pwa_fit_fractions.argtypes = [vp, dp, dp]
+    lib.pwa_nll_grad_for_hvp.argtypes = [vp, dp, dp, dp]
+    lib.pwa_hvp_cached.argtypes = [vp, dp, dp]
     lib.pwa_status_flags.argtypes = [vp, POINTER(c_uint32)]
     lib.pwa_profile_enable.argtypes = [vp, c_int32]
     lib.pwa_profile_read.argtypes = [vp, POINTER(c_double), POINTER(c_int64)]
@@ -251,6 +254,16 @@ def pwa_nll_grad_hvp_host(h, theta_host, v_host, nll_host, grad_host, hv_host) -
                                         _ptr(hv_host)), h)
 
 
+def pwa_nll_grad_for_hvp(h, theta, nll, grad) -> None:
+    P = pwa_n_params(h)
+    _check(load().pwa_nll_grad_for_hvp(h, _dev_f64(theta, P, "theta"), _dev_f64(nll, 1, "nll"), _dev_f64(grad, P, "grad")), h)
+
+
+def pwa_hvp_cached(h, v, hv) -> None:
+    P = pwa_n_params(h)
+    _check(load().pwa_hvp_cached(h, _dev_f64(v, P, "v"), _dev_f64(hv, P, "hv")), h)
+
+
 def pwa_fit_fractions(h, theta, frac) -> None:
     """frac[n_res] (device) <- fit fractions over the MC sample at theta (device)."""
     P = pwa_n_params(h)
@@ -333,6 +346,14 @@ class Model:
         raw = self.torch.zeros(4 + 4 * self.P, dtype=self.torch.float64, device=self.dev)
         pwa_raw_sums(self.h, self._d(theta), None if v is None else self._d(v), raw)
         return raw
+
+    def nll_grad_for_hvp(self, theta):
+        pwa_nll_grad_for_hvp(self.h, self._d(theta), self.nll_t, self.grad_t)
+        return self.nll_t.item(), self.grad_t.cpu().numpy().copy()
+
+    def hvp_cached(self, v):
+        pwa_hvp_cached(self.h, self._d(v), self.hv_t)
+        return self.hv_t.cpu().numpy().copy()
 
     def fit_fractions(self, theta):
         frac = self.torch.zeros(self.P // 4, dtype=self.torch.float64, device=self.dev)

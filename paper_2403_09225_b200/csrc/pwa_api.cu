@@ -81,7 +81,7 @@ static pwa_status raw_sums_impl(pwa_handle* h, int mode, const double* theta, co
   if (packed) {
     // lanes sweep: the per-resonance constants are formed by every block itself (no prologue launch)
     if (prof) cudaEventRecord(h->prof_events[h->prof_used], h->stream);
-    pwa_status st = lanes_launch(h, mode, theta, mode == MODE_FULL ? v : nullptr);
+    pwa_status st = lanes_launch(h, mode, theta, mode_q(mode) ? v : nullptr);
     if (st != PWA_OK) return st;
     h->launches++;
     if (prof) {
@@ -112,20 +112,18 @@ static pwa_status raw_sums_impl(pwa_handle* h, int mode, const double* theta, co
     if (cudaError_t ce = cudaGetLastError()) return set_error(h, PWA_ERR_CUDA, "launch sweep kernel", ce);
   }
   const double n_mc = (double)h->smp[0].n;
+#define PWA_REDUCE(M)                                                                                              \
+  k_reduce_unpack<M><<<kReduceBlocks, 1024, 0, h->stream>>>(h->d_partial, h->grid, nb, R, packed, theta, v, n_mc,  \
+                                                             h->d_sums, raw, combine ? 1 : 0, nll, grad, hv,        \
+                                                             h->d_flags, h->d_flags + 1, h->d_pcache)
   switch (mode) {
-    case MODE_NLL:
-      k_reduce_unpack<MODE_NLL><<<kReduceBlocks, 1024, 0, h->stream>>>(h->d_partial, h->grid, nb, R, packed, theta, v, n_mc, h->d_sums, raw,
-                                                             combine ? 1 : 0, nll, grad, hv, h->d_flags, h->d_flags + 1);
-      break;
-    case MODE_GRAD:
-      k_reduce_unpack<MODE_GRAD><<<kReduceBlocks, 1024, 0, h->stream>>>(h->d_partial, h->grid, nb, R, packed, theta, v, n_mc, h->d_sums, raw,
-                                                             combine ? 1 : 0, nll, grad, hv, h->d_flags, h->d_flags + 1);
-      break;
-    default:
-      k_reduce_unpack<MODE_FULL><<<kReduceBlocks, 1024, 0, h->stream>>>(h->d_partial, h->grid, nb, R, packed, theta, v, n_mc, h->d_sums, raw,
-                                                             combine ? 1 : 0, nll, grad, hv, h->d_flags, h->d_flags + 1);
-      break;
+    case MODE_NLL: PWA_REDUCE(MODE_NLL); break;
+    case MODE_GRAD: PWA_REDUCE(MODE_GRAD); break;
+    case MODE_GRAD3: PWA_REDUCE(MODE_GRAD3); break;
+    case MODE_HVPQ: PWA_REDUCE(MODE_HVPQ); break;
+    default: PWA_REDUCE(MODE_FULL); break;
   }
+#undef PWA_REDUCE
   h->launches++;
   if (cudaError_t ce = cudaGetLastError()) return set_error(h, PWA_ERR_CUDA, "launch k_reduce_unpack", ce);
   return PWA_OK;
@@ -142,6 +140,22 @@ static pwa_status combine_impl(pwa_handle* h, const double* raw, const double* v
 pwa_status eval(pwa_handle* h, int mode, const double* theta, const double* v, double* nll, double* grad, double* hv) {
   // sweep, then ONE launch for the second reduction stage, the unpacking and Eqs. 4, 6, 7
   return raw_sums_impl(h, mode, theta, v, h->d_raw, true, nll, grad, hv);
+}
+
+// Split evaluation for Newton-CG: the gradient call keeps theta and the direction-independent compact
+// sums P1, P2, P3 in the handle; every following HVP at that theta only accumulates Q1, Q2 (MODE_HVPQ).
+// Shapes served by the generic kernel have no such modes: they fall back to the fused sweep at the kept theta.
+pwa_status eval_grad_keep(pwa_handle* h, const double* theta, double* nll, double* grad) {
+  PWA_CUDA_CHECK(h, cudaMemcpyAsync(h->d_theta_keep, theta, sizeof(double) * h->n_par, cudaMemcpyDeviceToDevice, h->stream));
+  h->keep_valid = true;
+  if (h->variant < 2) return eval(h, MODE_GRAD, theta, nullptr, nll, grad, nullptr);
+  return raw_sums_impl(h, MODE_GRAD3, h->d_theta_keep, nullptr, h->d_raw, true, nll, grad, nullptr);
+}
+
+pwa_status eval_hvp_kept(pwa_handle* h, const double* v, double* hv) {
+  if (!h->keep_valid) return set_error(h, PWA_ERR_INVALID_ARG, "pwa_hvp_cached: no pwa_nll_grad_for_hvp call before", cudaSuccess);
+  if (h->variant < 2) return eval(h, MODE_FULL, h->d_theta_keep, v, nullptr, nullptr, hv);
+  return raw_sums_impl(h, MODE_HVPQ, h->d_theta_keep, v, h->d_raw, true, nullptr, nullptr, hv);
 }
 
 }  // namespace pwa
@@ -298,6 +312,8 @@ extern "C" pwa_status pwa_create(const pwa_model_desc* m, pwa_handle** out) {
             cudaMalloc(&h->d_sums, sizeof(double) * 2 * pstride) == cudaSuccess &&
             cudaMalloc(&h->d_raw, sizeof(double) * (4 + 4 * (size_t)P)) == cudaSuccess &&
             cudaMalloc(&h->d_flags, 2 * sizeof(unsigned)) == cudaSuccess &&
+            cudaMalloc(&h->d_pcache, sizeof(double) * 2 * (6 * (size_t)h->n_res + 2)) == cudaSuccess &&
+            cudaMalloc(&h->d_theta_keep, sizeof(double) * h->n_par) == cudaSuccess &&
             cudaMalloc(&h->d_io, sizeof(double) * io) == cudaSuccess &&
             cudaMalloc(&h->d_fit, sizeof(double) * (8 * (size_t)P + 64)) == cudaSuccess &&
             cudaMallocHost(&h->h_pin, sizeof(double) * io) == cudaSuccess &&
@@ -319,7 +335,7 @@ extern "C" pwa_status pwa_destroy(pwa_handle* h) {
   cudaSetDevice(h->device);
   cudaStreamSynchronize(h->stream);
   for (void* p : h->owned) if (p) cudaFree(p);
-  void* dev[] = {h->d_ch, h->d_K, h->d_partial, h->d_sums, h->d_raw, h->d_flags, h->d_io, h->d_fit};
+  void* dev[] = {h->d_ch, h->d_K, h->d_partial, h->d_sums, h->d_raw, h->d_flags, h->d_io, h->d_fit, h->d_pcache, h->d_theta_keep};
   for (void* p : dev) if (p) cudaFree(p);
   for (cudaEvent_t e : h->prof_events) cudaEventDestroy(e);
   if (h->h_pin) cudaFreeHost(h->h_pin);
@@ -440,6 +456,18 @@ extern "C" pwa_status pwa_profile_read(pwa_handle* h, double* total_ms, int64_t*
   if (n_launches) *n_launches = (int64_t)(h->prof_used / 2);
   h->prof_used = 0;
   return PWA_OK;
+}
+
+extern "C" pwa_status pwa_nll_grad_for_hvp(pwa_handle* h, const double* theta, double* nll, double* grad) {
+  if (!h) return PWA_ERR_INVALID_ARG;
+  if (!theta) return set_error(h, PWA_ERR_INVALID_ARG, "pwa_nll_grad_for_hvp: null theta", cudaSuccess);
+  return eval_grad_keep(h, theta, nll, grad);
+}
+
+extern "C" pwa_status pwa_hvp_cached(pwa_handle* h, const double* v, double* hv) {
+  if (!h) return PWA_ERR_INVALID_ARG;
+  if (!v || !hv) return set_error(h, PWA_ERR_INVALID_ARG, "pwa_hvp_cached: null pointer", cudaSuccess);
+  return eval_hvp_kept(h, v, hv);
 }
 
 extern "C" int64_t pwa_kernel_launches(const pwa_handle* h) { return h ? h->launches : -1; }

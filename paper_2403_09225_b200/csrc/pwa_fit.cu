@@ -188,7 +188,7 @@ extern "C" pwa_status pwa_fit_newton_cg(pwa_handle* h, double* theta, const pwa_
   } while (0)
 
   // step 1: f, g at theta
-  FIT_EVAL(pwa::eval(h, pwa::MODE_GRAD, theta, nullptr, sc + S_F, g, nullptr));
+  FIT_EVAL(pwa::eval_grad_keep(h, theta, sc + S_F, g));
   res->n_grad++;
   int stop = 0;
   double f = 0.0, ginf = 0.0;
@@ -213,7 +213,7 @@ extern "C" pwa_status pwa_fit_newton_cg(pwa_handle* h, double* theta, const pwa_
     // step 3: truncated CG on H p = -g
     bool have_p = false;
     for (int j = 0; j < o.max_cg; ++j) {
-      FIT_EVAL(pwa::eval(h, pwa::MODE_FULL, theta, d, nullptr, nullptr, q));
+      FIT_EVAL(pwa::eval_hvp_kept(h, d, q));
       res->n_hvp++;
       res->cg_iters++;
       k_cg_iter<<<1, FT, 0, st>>>(P, j, g, q, z, r, d, p, sc);
@@ -247,7 +247,7 @@ extern "C" pwa_status pwa_fit_newton_cg(pwa_handle* h, double* theta, const pwa_
     if (!accepted) { stop = 6; break; }
     // step 5: accept
     FIT_CHECK(cudaMemcpyAsync(theta, trial, sizeof(double) * P, cudaMemcpyDeviceToDevice, st));
-    FIT_EVAL(pwa::eval(h, pwa::MODE_GRAD, theta, nullptr, sc + S_F, g, nullptr));
+    FIT_EVAL(pwa::eval_grad_keep(h, theta, sc + S_F, g));
     res->n_grad++;
     const bool small_step = t * pinf <= o.xtol;
     const bool small_df = std::fabs(fnew - f) <= o.ftol * std::fmax(1.0, std::fabs(f));

@@ -28,6 +28,9 @@ struct pwa_handle {
   double* d_raw = nullptr;      // public raw vector (4 + 4P)
   unsigned* d_flags = nullptr;  // [0] non-finite flag of the last evaluation, [1] ticket counter of the reduction kernel
   size_t partial_doubles = 0;
+  double* d_pcache = nullptr;      // [2][6 R + 2] compact sums P1..P3 + scalars of the last pwa_nll_grad_for_hvp
+  double* d_theta_keep = nullptr;  // theta of that call
+  bool keep_valid = false;
 
   // sweep launch configuration (fixed at creation -> deterministic event -> thread map)
   int grid = 0, block = 0;
@@ -37,6 +40,7 @@ struct pwa_handle {
   pwa::LaneArgs largs;
   size_t lanes_smem = 0;
   int lanes_combo = -1;
+  int lanes_combo_alt = -1, block_alt = 0;  // shape of the gradient modes (MODE_GRAD, MODE_GRAD3), if another one
   bool weight_padded = false;  // the data weights are library-owned and padded to an even length
 
   // device staging for the *_host entry point and the fit driver
@@ -61,14 +65,17 @@ bool encode_2d(CUtensorMap* m, const void* base, unsigned long long cols, unsign
 // pwa_sweep_lanes.cu
 typedef void (*lanes_fn)(const LaneArgs);
 struct LanesCombo {
-  int rho, log_sw, nw, prod, tile;  // resonances per lane, log2(slices per warp), compute warps per block, producer kind
-                                    // (0 warp, 2 warpgroup), events per tile (32, or 8 with the swizzled layout)
+  int rho, log_sw, nw, prod, tile, alt;  // resonances per lane, log2(slices per warp), compute warps per block, producer kind
+                                    // (0 warp, 2 warpgroup), events per tile (32, or 8 with the swizzled layout), and the
+                                    // entry (same rho, slices, tile) used for the gradient modes, whose registers allow a
+                                    // third compute warp per scheduler (-1: none)
 };
 // instantiated shapes (pwa_sweep_lanes_inst.cu); capacity RHO << LOG_SW resonances; the handle takes the first entry of
 // the smallest capacity >= R whose stages fit in shared memory at least twice
-constexpr LanesCombo kLanesCombos[] = {{1, 2, 15, 0, 32}, {2, 3, 15, 0, 32}, {3, 2, 11, 0, 32}, {3, 2, 8, 2, 32}, {4, 3, 8, 2, 32},
-                                       {4, 3, 7, 0, 32}, {4, 4, 8, 2, 32}, {4, 4, 7, 0, 32}, {4, 5, 8, 2, 32}, {4, 5, 7, 0, 32},
-                                       {4, 4, 8, 2, 8}, {4, 5, 8, 2, 8}};
+constexpr LanesCombo kLanesCombos[] = {
+    {1, 2, 15, 0, 32, -1}, {2, 3, 15, 0, 32, -1}, {3, 2, 11, 0, 32, -1}, {3, 2, 8, 2, 32, -1}, {4, 3, 8, 2, 32, 12}, {4, 3, 7, 0, 32, -1},
+    {4, 4, 8, 2, 32, -1},  {4, 4, 7, 0, 32, -1},  {4, 5, 8, 2, 32, -1},  {4, 5, 7, 0, 32, -1}, {4, 4, 8, 2, 8, -1},  {4, 5, 8, 2, 8, -1},
+    {4, 3, 11, 3, 32, -1}};
 constexpr int kNumLanesCombos = sizeof(kLanesCombos) / sizeof(kLanesCombos[0]);
 lanes_fn lanes_kernel_h1(int combo, int mode);
 lanes_fn lanes_kernel_h2(int combo, int mode);
@@ -80,6 +87,8 @@ pwa_status lanes_launch(pwa_handle* h, int mode, const double* theta, const doub
 // internal entry points used by the fit driver (enqueue only)
 pwa_status eval(pwa_handle* h, int mode, const double* theta, const double* v, double* nll, double* grad,
                 double* hv);
+pwa_status eval_grad_keep(pwa_handle* h, const double* theta, double* nll, double* grad);
+pwa_status eval_hvp_kept(pwa_handle* h, const double* v, double* hv);
 pwa_status set_error(pwa_handle* h, pwa_status st, const char* what, cudaError_t ce);
 }  // namespace pwa
 

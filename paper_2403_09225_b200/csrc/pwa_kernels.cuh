@@ -358,7 +358,7 @@ __global__ void __launch_bounds__(1024) k_reduce_unpack(const double* __restrict
                                                         const double* __restrict__ v, double n_mc, double* sums, double* raw,
                                                         int combine, double* __restrict__ nll, double* __restrict__ grad,
                                                         double* __restrict__ hv, unsigned* __restrict__ flags,
-                                                        unsigned* ticket) {
+                                                        unsigned* ticket, double* pcache) {
   constexpr int VPR = vpr_of(MODE), RPB = rpb_of(MODE);
   const int nacc = packed ? (MODE == MODE_NLL ? 0 : R * VPR) : nb * 32, stride = nacc + 2, P = 4 * R;
   // Phase 1 over all blocks of this launch: block g sums the columns k = g * 1024 + t, (g + gridDim) * 1024 + t, ...
@@ -397,10 +397,17 @@ __global__ void __launch_bounds__(1024) k_reduce_unpack(const double* __restrict
   } else {
     __syncthreads();
   }
+  // MODE_GRAD3 leaves its block-summed compact sums (P1, P2, P3 and the scalars) in pcache: [2][6 R + 2];
+  // MODE_HVPQ takes P1..P3 and the scalars from there and only Q1, Q2 from this sweep.
+  const int cstride = 6 * R + 2;
+  if (MODE == MODE_GRAD3)
+    for (int k = threadIdx.x; k < 2 * stride; k += blockDim.x) pcache[k] = __ldcg(sums + k);
+  const double* sc = MODE == MODE_HVPQ ? pcache : sums;   // where the scalars and the P sums live
+  const int sstride = MODE == MODE_HVPQ ? cstride : stride, snacc = MODE == MODE_HVPQ ? 6 * R : nacc;
   if (threadIdx.x == 0) {
-    raw[0] = __ldcg(sums + stride + nacc);      // sum_data w ln I
-    raw[1] = __ldcg(sums + stride + nacc + 1);  // W
-    raw[2] = __ldcg(sums + nacc);               // G
+    raw[0] = __ldcg(sc + sstride + snacc);      // sum_data w ln I
+    raw[1] = __ldcg(sc + sstride + snacc + 1);  // W
+    raw[2] = __ldcg(sc + snacc);                // G
     raw[3] = n_mc;
   }
   if (MODE == MODE_NLL) {
@@ -413,17 +420,25 @@ __global__ void __launch_bounds__(1024) k_reduce_unpack(const double* __restrict
       for (int sample = 0; sample < 2; ++sample) {
         const double* q = sums + (size_t)sample * stride + qoff;
         Sums5 s;
-        s.P1 = {__ldcg(q), __ldcg(q + 1)};
-        s.P2 = {__ldcg(q + 2), __ldcg(q + 3)};
-        if (MODE == MODE_FULL) {
-          s.P3 = {__ldcg(q + 4), __ldcg(q + 5)};
-          s.Q1 = {__ldcg(q + 6), __ldcg(q + 7)};
-          s.Q2 = {__ldcg(q + 8), __ldcg(q + 9)};
+        s.P3 = s.Q1 = s.Q2 = {0.0, 0.0};
+        if (MODE == MODE_HVPQ) {
+          const double* pc = pcache + (size_t)sample * cstride + r * 6;
+          s.P1 = {__ldcg(pc), __ldcg(pc + 1)};
+          s.P2 = {__ldcg(pc + 2), __ldcg(pc + 3)};
+          s.P3 = {__ldcg(pc + 4), __ldcg(pc + 5)};
+          s.Q1 = {__ldcg(q), __ldcg(q + 1)};
+          s.Q2 = {__ldcg(q + 2), __ldcg(q + 3)};
         } else {
-          s.P3 = s.Q1 = s.Q2 = {0.0, 0.0};
+          s.P1 = {__ldcg(q), __ldcg(q + 1)};
+          s.P2 = {__ldcg(q + 2), __ldcg(q + 3)};
+          if (MODE == MODE_FULL || MODE == MODE_GRAD3) s.P3 = {__ldcg(q + 4), __ldcg(q + 5)};
+          if (MODE == MODE_FULL) {
+            s.Q1 = {__ldcg(q + 6), __ldcg(q + 7)};
+            s.Q2 = {__ldcg(q + 8), __ldcg(q + 9)};
+          }
         }
         double g4[4], h4[4] = {0.0, 0.0, 0.0, 0.0};
-        unpack_res(s, a, phi, M, G, (MODE == MODE_FULL && v) ? v + 4 * r : nullptr, g4, h4);
+        unpack_res(s, a, phi, M, G, (mode_q(MODE) && v) ? v + 4 * r : nullptr, g4, h4);
         // raw layout: gd | gG | hd | hG ; data (sample 1) carries hd = -h
         double* gdst = raw + 4 + (sample == 1 ? 0 : P) + 4 * r;
         double* hdst = raw + 4 + 2 * P + (sample == 1 ? 0 : P) + 4 * r;
@@ -436,7 +451,7 @@ __global__ void __launch_bounds__(1024) k_reduce_unpack(const double* __restrict
   }
   if (combine) {
     __syncthreads();  // the raw vector of this block's own writes is visible to the whole block
-    combine_block(raw, (MODE == MODE_FULL) ? v : nullptr, P, nll, grad, (MODE == MODE_FULL) ? hv : nullptr, flags);
+    combine_block(raw, mode_q(MODE) ? v : nullptr, P, nll, grad, mode_q(MODE) ? hv : nullptr, flags);
   }
 }
 

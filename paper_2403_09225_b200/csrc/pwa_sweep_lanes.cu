@@ -101,18 +101,19 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
       if (cap < R || !lanes_kernel(H, k, MODE_FULL)) continue;
       rho = c.rho; log_sw = c.log_sw; nw = c.nw; prod = c.prod; tile = c.tile;
       nthreads = lanes::lanes_threads(nw, prod);
-      SW = 1 << log_sw; RP = rho * SW; NW = nw;
+      SW = 1 << log_sw; RP = rho * SW;
+      NW = c.alt >= 0 ? std::max(nw, kLanesCombos[c.alt].nw) : nw;  // per-warp scratch sized for the larger of the two shapes
       if (tile == 32) {
         // amplitude rows incl. the zero-filled planes of padding resonances, in nbox boxes of rows_box (<= 256) rows
         const int rows_need = RP * H;
         nbox = (rows_need + 255) / 256; rows_box = (rows_need + nbox - 1) / nbox;
         amp_bytes = (unsigned)nbox * rows_box * tile * 16;
-        red_bytes = up((unsigned)NW * (R * 10 + 2) * 8, 128);
+        red_bytes = up((unsigned)nw * (R * 10 + 2) * 8, 128);  // rows for the main shape's warps only
       } else {
         if (RP > 256) continue;  // one 3-D box [H][RP][8 events]
         nbox = 1; rows_box = RP;
         amp_bytes = (unsigned)H * RP * tile * 16;
-        red_bytes = 0;  // the warps add into the block's partial row in turn
+        red_bytes = up((unsigned)(R * 10 + 2) * 8, 128);  // one row: the warps add into it in turn
       }
       off_mass = amp_bytes; off_wgt = up(off_mass + (unsigned)C * tile * 8, 128);  // TMA destinations: 128-byte aligned
       stage_bytes = up(off_wgt + tile * 8, tile == 32 ? 128 : 1024);
@@ -131,12 +132,15 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
   why.clear();
   const size_t smem = (size_t)stages * stage_bytes + fixed;
 
-  for (int mode = 0; mode < 3; ++mode) {
-    lanes_fn fn = lanes_kernel(H, combo, mode);
+  for (int mode = 0; mode < 5; ++mode) {
+    const bool use_alt = kLanesCombos[combo].alt >= 0 && (mode == MODE_GRAD || mode == MODE_GRAD3);
+    const int cmb = use_alt ? kLanesCombos[combo].alt : combo;
+    const int nthr = lanes::lanes_threads(kLanesCombos[cmb].nw, kLanesCombos[cmb].prod);
+    lanes_fn fn = lanes_kernel(H, cmb, mode);
     cudaError_t ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, dev_smem);
     if (ce != cudaSuccess) return set_error(h, PWA_ERR_CUDA, "cudaFuncSetAttribute(lanes sweep)", ce);
     int occ = 0;
-    ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, nthreads, smem);
+    ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, nthr, smem);
     if (ce != cudaSuccess || occ < 1) {
       cudaGetLastError();
       why = "lanes kernel cannot be resident (registers / shared memory)";
@@ -176,10 +180,13 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
   a.off_bar = a.off_xch + xch_bytes;
   h->lanes_smem = smem;
   h->lanes_combo = combo;
+  h->lanes_combo_alt = kLanesCombos[combo].alt;
+  if (h->lanes_combo_alt >= 0)
+    h->block_alt = lanes::lanes_threads(kLanesCombos[h->lanes_combo_alt].nw, kLanesCombos[h->lanes_combo_alt].prod);
   h->variant = 2;
   h->block = nthreads;
   h->grid = h->num_sms;
-  std::snprintf(h->variant_name, sizeof(h->variant_name), "lanes(rho=%d,sw=%d,nw=%d%s,tile=%d,stages=%d)", rho, SW, NW, prod == 2 ? "g" : "", tile, stages);
+  std::snprintf(h->variant_name, sizeof(h->variant_name), "lanes(rho=%d,sw=%d,nw=%d%s,tile=%d,stages=%d)", rho, SW, nw, prod == 2 ? "g" : "", tile, stages);
   return PWA_OK;
 }
 
@@ -188,8 +195,9 @@ pwa_status lanes_launch(pwa_handle* h, int mode, const double* theta, const doub
   a.theta = theta;
   a.v = v;
   a.partial = h->d_partial;
-  lanes_fn fn = lanes_kernel(h->n_hel, h->lanes_combo, mode);
-  fn<<<h->grid, h->block, h->lanes_smem, h->stream>>>(a);
+  const bool use_alt = h->lanes_combo_alt >= 0 && (mode == MODE_GRAD || mode == MODE_GRAD3);
+  lanes_fn fn = lanes_kernel(h->n_hel, use_alt ? h->lanes_combo_alt : h->lanes_combo, mode);
+  fn<<<h->grid, use_alt ? h->block_alt : h->block, h->lanes_smem, h->stream>>>(a);
   if (cudaError_t ce = cudaGetLastError()) return set_error(h, PWA_ERR_CUDA, "launch lanes sweep kernel", ce);
   return PWA_OK;
 }

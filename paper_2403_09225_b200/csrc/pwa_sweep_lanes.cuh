@@ -213,7 +213,7 @@ __device__ __forceinline__ void resonance_constants(const double* __restrict__ t
 
 template <int MODE>
 __host__ __device__ constexpr int nacc_of() {
-  return MODE == MODE_FULL ? 10 : (MODE == MODE_GRAD ? 4 : 0);
+  return MODE == MODE_NLL ? 0 : vpr_of(MODE);
 }
 // NW compute warps + 1 producer warp per block; (NW + 1) / 4 warps share one SM sub-partition's 16 K registers,
 // so NW = 7 / 11 / 15 allows 255 / 168 / 128 registers per thread.
@@ -223,6 +223,8 @@ __host__ __device__ constexpr int nacc_of() {
 //   0  warp NW is a dedicated producer (NW + 1 warps; with NW = 7 one SM sub-partition has a single compute warp);
 //      (a variant without any producer warp, the compute warp of column 0 issuing the copies, was measured slower:
 //      the feed then waits for that warp's turn);
+//   3  as 0, but without per-warp reduction rows in shared memory (the warps add into the block's partial row in
+//      turn): the shape a handle uses for its gradient modes beside its main shape, whose scratch it shares;
 //   2  producer warpgroup: warps 0..3 shrink to 24 registers (setmaxnreg.dec), warp 0 produces; the NW compute warps
 //      4..NW+3 grow to 240 registers (setmaxnreg.inc), so every sub-partition carries NW / 4 compute warps.
 constexpr int lanes_threads(int nw, int prod) { return (nw + (prod == 2 ? 4 : 1)) * 32; }
@@ -240,7 +242,9 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
   constexpr int EW = 32 / SW;              // events per pass
   constexpr int NP = TILE / EW;            // passes per tile
   static_assert(TILE == 32 || (TILE == 8 && SW >= 8), "8-event tiles need at least 8 slices (swizzle phase = slice & 7)");
-  constexpr int NV = (MODE == MODE_FULL ? 4 : 2) * H;  // reals exchanged per event and slice
+  constexpr bool WP = mode_p(MODE), WP3 = mode_p3(MODE), WQ = mode_q(MODE);
+  constexpr int QO = MODE == MODE_FULL ? 6 : 0;  // first accumulator of Q1 (FULL: after P1..P3; HVPQ: the only ones)
+  constexpr int NV = (WQ ? 4 : 2) * H;  // reals exchanged per event and slice
   constexpr int NACC = nacc_of<MODE>();
   constexpr int NA = NACC > 0 ? NACC : 1;
   constexpr int RP = RHO * SW;             // resonances incl. padding
@@ -255,7 +259,7 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
   for (int r = threadIdx.x; r < RP; r += blockDim.x) {
     double* k = Ks + r * KS;
     if (r < R) {
-      resonance_constants(a.theta, MODE == MODE_FULL ? a.v : nullptr, r, (long long)a.off_mass + (long long)a.ch[r] * (TILE * 8), k);
+      resonance_constants(a.theta, WQ ? a.v : nullptr, r, (long long)a.off_mass + (long long)a.ch[r] * (TILE * 8), k);
     } else {  // padding resonance: couples to nothing, propagator finite
       k[0] = 0.0; k[1] = 1.0; k[2] = 0.0; k[3] = __longlong_as_double((long long)a.off_mass);
       k[4] = k[5] = k[6] = k[7] = k[8] = k[9] = 0.0;
@@ -296,9 +300,9 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
     tma_load_2d(dst + a.off_mass, &a.tm_mass[smp], i0, 0, bar);
     if (wg) tma_load_2d(dst + a.off_wgt, &a.tm_wgt[smp], i0, 0, bar);
   };
-  if ((PROD == 0 && w == NW) || (PROD == 2 && w < 0)) {
+  if ((PROD != 2 && w == NW) || (PROD == 2 && w < 0)) {
     if (PROD == 2) asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
-    if (lane == 0 && (PROD == 0 || w == -4) && !kNoLoad) {
+    if (lane == 0 && (PROD != 2 || w == -4) && !kNoLoad) {
       tma_prefetch_desc(&a.tm_amp[0]);
       tma_prefetch_desc(&a.tm_mass[0]);
       tma_prefetch_desc(&a.tm_amp[1]);
@@ -407,7 +411,7 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
           }
         } else {
           double wr = 0.0, wi = 0.0;
-          if (MODE == MODE_FULL) {  // zdot = (alpha + beta B) B
+          if (WQ) {  // zdot = (alpha + beta B) B
             const double2 al = kk[3], be = kk[4];
             wr = fma(be.x, br, fma(-be.y, bi, al.x));
             wi = fma(be.x, bi, fma(be.y, br, al.y));
@@ -420,14 +424,14 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
             if (j == 0) {
               x[2 * h] = fma(c.x, gx, -(c.y * gy));
               x[2 * h + 1] = fma(c.x, gy, c.y * gx);
-              if (MODE == MODE_FULL) {
+              if (WQ) {
                 x[2 * H + 2 * h] = fma(wr, gx, -(wi * gy));
                 x[2 * H + 2 * h + 1] = fma(wr, gy, wi * gx);
               }
             } else {
               x[2 * h] = fma(c.x, gx, fma(-c.y, gy, x[2 * h]));
               x[2 * h + 1] = fma(c.x, gy, fma(c.y, gx, x[2 * h + 1]));
-              if (MODE == MODE_FULL) {
+              if (WQ) {
                 x[2 * H + 2 * h] = fma(wr, gx, fma(-wi, gy, x[2 * H + 2 * h]));
                 x[2 * H + 2 * h + 1] = fma(wr, gy, fma(wi, gx, x[2 * H + 2 * h + 1]));
               }
@@ -461,10 +465,10 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
         const double Iv = valid ? I : 1.0;
         const double inv = 1.0 / Iv;
         const double om = wv * inv;
-        s0 = fma(wv, log(Iv), s0);
+        if (MODE != MODE_HVPQ) s0 = fma(wv, log(Iv), s0);  // HVPQ: the scalars come from the cached gradient evaluation
         s1 += wv;
         double kap = 0.0;
-        if (MODE == MODE_FULL) {
+        if (WQ) {
           double Idot = 0.0;
 #pragma unroll
           for (int h = 0; h < H; ++h)
@@ -473,7 +477,7 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
         }
 #pragma unroll
         for (int h = 0; h < H; ++h) {
-          if (MODE == MODE_FULL) {
+          if (WQ) {
             x[2 * H + 2 * h] = om * fma(-kap, x[2 * h], x[2 * H + 2 * h]);
             x[2 * H + 2 * h + 1] = om * fma(-kap, x[2 * h + 1], x[2 * H + 2 * h + 1]);
           }
@@ -487,42 +491,49 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
 #pragma unroll
         for (int j = 0; j < RHO; ++j) {
           const double br = Br[j].x, bi = Br[j].y;
-          // t1 = B S = sum_h conj(A_h) G_h ;  u1 = B S' = sum_h conj(D_h) G_h
-          double t1r, t1i, u1r = 0.0, u1i = 0.0;
-          {
-            const double2 g = Gr[j][0];
-            t1r = fma(x[0], g.x, x[1] * g.y);
-            t1i = fma(x[0], g.y, -(x[1] * g.x));
-            if (MODE == MODE_FULL) {
+          if (WP) {  // t1 = B S = sum_h conj(A_h) G_h
+            double t1r, t1i;
+            {
+              const double2 g = Gr[j][0];
+              t1r = fma(x[0], g.x, x[1] * g.y);
+              t1i = fma(x[0], g.y, -(x[1] * g.x));
+            }
+#pragma unroll
+            for (int h = 1; h < H; ++h) {
+              const double2 g = Gr[j][h];
+              t1r = fma(x[2 * h], g.x, fma(x[2 * h + 1], g.y, t1r));
+              t1i = fma(x[2 * h], g.y, fma(-x[2 * h + 1], g.x, t1i));
+            }
+            acc[j][0] += t1r;  // P1
+            acc[j][1] += t1i;
+            if (!WP3) {
+              acc[j][2] = fma(br, t1r, fma(-bi, t1i, acc[j][2]));  // P2
+              acc[j][3] = fma(br, t1i, fma(bi, t1r, acc[j][3]));
+            } else {
+              const double t2r = fma(br, t1r, -(bi * t1i)), t2i = fma(br, t1i, bi * t1r);
+              acc[j][2] += t2r;  // P2
+              acc[j][3] += t2i;
+              acc[j][4] = fma(br, t2r, fma(-bi, t2i, acc[j][4]));  // P3
+              acc[j][5] = fma(br, t2i, fma(bi, t2r, acc[j][5]));
+            }
+          }
+          if (WQ) {  // u1 = B S' = sum_h conj(omega (Adot_h - kappa A_h)) G_h
+            double u1r, u1i;
+            {
+              const double2 g = Gr[j][0];
               u1r = fma(x[2 * H], g.x, x[2 * H + 1] * g.y);
               u1i = fma(x[2 * H], g.y, -(x[2 * H + 1] * g.x));
             }
-          }
 #pragma unroll
-          for (int h = 1; h < H; ++h) {
-            const double2 g = Gr[j][h];
-            t1r = fma(x[2 * h], g.x, fma(x[2 * h + 1], g.y, t1r));
-            t1i = fma(x[2 * h], g.y, fma(-x[2 * h + 1], g.x, t1i));
-            if (MODE == MODE_FULL) {
+            for (int h = 1; h < H; ++h) {
+              const double2 g = Gr[j][h];
               u1r = fma(x[2 * H + 2 * h], g.x, fma(x[2 * H + 2 * h + 1], g.y, u1r));
               u1i = fma(x[2 * H + 2 * h], g.y, fma(-x[2 * H + 2 * h + 1], g.x, u1i));
             }
-          }
-          acc[j][0] += t1r;  // P1
-          acc[j][1] += t1i;
-          if (MODE == MODE_GRAD) {
-            acc[j][2] = fma(br, t1r, fma(-bi, t1i, acc[j][2]));  // P2
-            acc[j][3] = fma(br, t1i, fma(bi, t1r, acc[j][3]));
-          } else {
-            const double t2r = fma(br, t1r, -(bi * t1i)), t2i = fma(br, t1i, bi * t1r);
-            acc[j][2] += t2r;  // P2
-            acc[j][3] += t2i;
-            acc[j][4] = fma(br, t2r, fma(-bi, t2i, acc[j][4]));  // P3
-            acc[j][5] = fma(br, t2i, fma(bi, t2r, acc[j][5]));
-            acc[j][6] += u1r;  // Q1
-            acc[j][7] += u1i;
-            acc[j][8] = fma(br, u1r, fma(-bi, u1i, acc[j][8]));  // Q2
-            acc[j][9] = fma(br, u1i, fma(bi, u1r, acc[j][9]));
+            acc[j][QO] += u1r;  // Q1
+            acc[j][QO + 1] += u1i;
+            acc[j][QO + 2] = fma(br, u1r, fma(-bi, u1i, acc[j][QO + 2]));  // Q2
+            acc[j][QO + 3] = fma(br, u1i, fma(bi, u1r, acc[j][QO + 3]));
           }
         }
       }
@@ -543,7 +554,7 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
     //      partial row per block --------------------------------------------------------------------------------
     const int row_len = R * NACC + 2;
     double* out = a.partial + ((size_t)smp * gridDim.x + blockIdx.x) * (size_t)row_len;
-    if (TILE == 32) {
+    if (TILE == 32 && PROD != 3) {
       double* mine = red + (size_t)w * row_len;
 #pragma unroll
       for (int j = 0; j < RHO; ++j) {
@@ -578,10 +589,9 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
       }
       asm volatile("bar.sync 1, %0;" ::"n"(NW * 32) : "memory");
     } else {
-      // large shapes keep no per-warp rows in shared memory: the warps add into the block's partial row in turn
-      // (warp 0 writes, warp 1 adds, ...; the same fixed order, one named barrier per turn)
+      // no per-warp rows in shared memory (large shapes, or a shape with more warps than the handle's main one):
+      // ONE row in shared memory: warp 0 writes it, warp 1 adds, ... (fixed order, one named barrier per turn)
 #pragma unroll 1
-      volatile double* outv = out;  // read back what the previous warp wrote, not a cached copy
       for (int turn = 0; turn < NW; ++turn) {
         if (w == turn) {
 #pragma unroll
@@ -592,7 +602,7 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
               double tsum = acc[j][q];
 #pragma unroll
               for (int m = 1; m < EW; m <<= 1) tsum += shfl_x(tsum, m);
-              if (e == 0 && r < R) outv[r * NACC + q] = turn == 0 ? tsum : outv[r * NACC + q] + tsum;
+              if (e == 0 && r < R) red[r * NACC + q] = turn == 0 ? tsum : red[r * NACC + q] + tsum;
               acc[j][q] = 0.0;
             }
           }
@@ -603,14 +613,15 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
             t1 += shfl_x(t1, m);
           }
           if (lane == 0) {
-            outv[R * NACC] = turn == 0 ? t0 : outv[R * NACC] + t0;
-            outv[R * NACC + 1] = turn == 0 ? t1 : outv[R * NACC + 1] + t1;
+            red[R * NACC] = turn == 0 ? t0 : red[R * NACC] + t0;
+            red[R * NACC + 1] = turn == 0 ? t1 : red[R * NACC + 1] + t1;
           }
           s0 = s1 = 0.0;
-          __threadfence_block();
         }
         asm volatile("bar.sync 1, %0;" ::"n"(NW * 32) : "memory");
       }
+      for (int k = w * 32 + lane; k < row_len; k += NW * 32) out[k] = red[k];
+      asm volatile("bar.sync 1, %0;" ::"n"(NW * 32) : "memory");
     }
   }
 }

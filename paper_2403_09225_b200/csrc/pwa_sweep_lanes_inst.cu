@@ -13,6 +13,8 @@ lanes_fn for_mode(int mode) {
   switch (mode) {
     case MODE_NLL: return lanes::k_sweep_lanes<PWA_LANES_H, RHO, LOG_SW, NW, MODE_NLL, PROD, TILE>;
     case MODE_GRAD: return lanes::k_sweep_lanes<PWA_LANES_H, RHO, LOG_SW, NW, MODE_GRAD, PROD, TILE>;
+    case MODE_GRAD3: return lanes::k_sweep_lanes<PWA_LANES_H, RHO, LOG_SW, NW, MODE_GRAD3, PROD, TILE>;
+    case MODE_HVPQ: return lanes::k_sweep_lanes<PWA_LANES_H, RHO, LOG_SW, NW, MODE_HVPQ, PROD, TILE>;
     default: return lanes::k_sweep_lanes<PWA_LANES_H, RHO, LOG_SW, NW, MODE_FULL, PROD, TILE>;
   }
 }
@@ -34,6 +36,7 @@ lanes_fn PWA_CAT(lanes_kernel_h, PWA_LANES_H)(int combo, int mode) {
     case 9: return for_mode<4, 5, 7>(mode);
     case 10: return for_mode<4, 4, 8, 2, 8>(mode);
     case 11: return for_mode<4, 5, 8, 2, 8>(mode);
+    case 12: return for_mode<4, 3, 11, 3>(mode);
   }
   return nullptr;
 }

@@ -265,3 +265,37 @@ def test_fit_fractions_match_oracle(pwa, oracle_mod, idx, n_mc, n_data):
         assert f.shape == f0.shape and np.all(np.isfinite(f))
         assert np.max(np.abs(f - f0) / f0) < 1e-10, idx
         assert gm.fit_fractions(th).tobytes() == f.tobytes()  # repeat runs bit-identical
+
+
+@pytest.mark.parametrize("idx,n_mc,n_data", CASES)
+def test_split_evaluation_matches_oracle(pwa, oracle_mod, idx, n_mc, n_data):
+    """pwa_nll_grad_for_hvp + pwa_hvp_cached (the Newton-CG split of include/pwa.h) against the oracle: NLL and
+    gradient from the keeping call, then several HVPs at the kept theta with other calls in between."""
+    import workloads
+    cfg, w, om, gm = _case(pwa, oracle_mod, idx, n_mc, n_data)
+    for k, th in enumerate(_thetas(cfg)[:2]):
+        f0, g0, _ = oracle_mod.nll_grad_hvp(om, th, None, "ld")
+        f, g = gm.nll_grad_for_hvp(th)
+        assert _nll_err(f, f0) < NLL_TOL and rel_l2(g, g0) < VEC_TOL
+        other = _thetas(cfg)[3]
+        for j in range(3):
+            v = workloads.direction(cfg, 10 + j).numpy()
+            h0 = oracle_mod.nll_grad_hvp(om, th, v, "ld")[2]
+            hv = gm.hvp_cached(v)
+            assert rel_l2(hv, h0) < VEC_TOL, (idx, k, j)
+            assert rel_l2(hv, gm.hvp(th, v)) < 1e-12           # same sums, other association
+            gm.nll(other); gm.nll_grad(other)                    # what is kept survives other evaluations
+            assert gm.hvp_cached(v).tobytes() == hv.tobytes()
+        assert pwa.pwa_status_flags(gm.h) == 0
+
+
+def test_hvp_cached_needs_a_keeping_call(pwa, oracle_mod):
+    import workloads
+    cfg, w, om, _ = _case(pwa, oracle_mod, *CASES[0])
+    gm = pwa.Model(w)
+    try:
+        with pytest.raises(pwa.PwaError) as e:
+            gm.hvp_cached(workloads.direction(cfg, 0).numpy())
+        assert e.value.status == 1
+    finally:
+        gm.close()
