@@ -2,7 +2,7 @@
 //
 // Work decomposition.  A tile is 32 consecutive events.  Tiles reach shared memory through a ring of stages
 // filled by one producer thread with TMA tensor copies (cp.async.bulk.tensor.2d): one box of 32 events x all R*H
-// amplitude planes (512 contiguous bytes per plane; narrower boxes were measured to cap the feed at 4.5 TB/s), one
+// amplitude planes (512 contiguous bytes per plane; narrower boxes were measured to cap the feed near 4.1 TB/s), one
 // box for the mass planes, one for the weights; full[stage] / empty[stage] mbarriers track the ring; events beyond
 // the ragged end and the planes of padding resonances are zero-filled by the TMA unit.  Every F element is read
 // from HBM exactly once and is consumed by exactly one thread.
@@ -12,12 +12,12 @@
 // r = j * SW + s, j < RHO.  Per pass a lane
 //   forward : B_r = 1/D_r (a-1), G_rh = B_r F_rh, slice-partial A_h = sum c_r G_rh, Adot_h = sum (alpha_r + beta_r B_r) G_rh
 //             (a-2); F is now in registers, the stage is released
-//   exchange: the 2H (4H with the HVP) real partials are summed over the SW slices INSIDE THE WARP by a
-//             reduce-scatter / all-gather over the slice bits of the lane id (shuffles; no shared memory, no
-//             barrier, fixed order)
+//   exchange: the 2H (4H with the HVP) real partials are summed over the SW slices INSIDE THE WARP: a shuffle
+//             reduce-scatter over the slice bits of the lane id, then every lane stores the total it holds into the
+//             warp's exchange row and reads all of them back (__syncwarp only; fixed order)
 //   event   : I = sum |A_h|^2; data: ln I, omega = w / I, kappa = Idot / I  (a-3, a-4)
 //   backward: B S_r = sum_h conj(omega A_h) G_rh, B S'_r = sum_h conj(omega (Adot_h - kappa A_h)) G_rh, and from them the
-//             five compact sums P1, P2, P3, Q1, Q2 of pwa_common.cuh (a-5, a-6) in per-lane registers
+//             compact sums P1, P2, P3, Q1, Q2 of pwa_common.cuh (a-5, a-6; which of them: the MODE) in per-lane registers
 // Warps never wait for one another: the only synchronisation inside the tile loop is the TMA ring.  At the end of
 // each sample the accumulators are summed over the event lanes (butterfly), over the warps of the block (shared
 // memory, fixed order) and written as one partial row per block (a-7, first stage).
