@@ -314,17 +314,41 @@ def main():
         ms = float(t.item())
     nll_dev = m.nll_t.item()
 
-    # ---- end to end through the host-buffer entry point: H2D of theta, v and D2H of nll, grad, hv every step ----
+    # ---- end to end: H2D of theta, v (pinned) and D2H of nll, grad, hv every step, synchronised ----
+    # one GPU: the library's host-buffer entry point; several: the same copies around raw sums -> all-reduce -> combine
     th_h, v_h = np.ascontiguousarray(th_np), np.ascontiguousarray(v_np)
     o_nll, o_g, o_h = np.zeros(1), np.zeros(P), np.zeros(P)
+    sharded_e2e = world > 1 or os.environ.get("PWA_BENCH_FORCE_SHARDED_E2E") == "1"
+    if sharded_e2e:
+        pin_in = torch.empty(2 * P, dtype=torch.float64).pin_memory()
+        pin_in[:P] = torch.from_numpy(th_h)
+        pin_in[P:] = torch.from_numpy(v_h)
+        pin_out = torch.empty(1 + 2 * P, dtype=torch.float64).pin_memory()
+        d_in = torch.empty(2 * P, dtype=torch.float64, device=dev)
+        d_out = torch.empty(1 + 2 * P, dtype=torch.float64, device=dev)
+
+    def e2e_step():
+        if not sharded_e2e:
+            pwa.pwa_nll_grad_hvp_host(m.h, th_h, v_h, o_nll, o_g, o_h)
+            return
+        d_in.copy_(pin_in, non_blocking=True)
+        pwa.pwa_raw_sums(m.h, d_in[:P], d_in[P:], raw)
+        if world > 1:
+            dist.all_reduce(raw)
+        pwa.pwa_combine(m.h, raw, d_in[P:], d_out[0:1], d_out[1:1 + P], d_out[1 + P:])
+        pin_out.copy_(d_out, non_blocking=True)
+        torch.cuda.synchronize()
+
     for _ in range(2):
-        pwa.pwa_nll_grad_hvp_host(m.h, th_h, v_h, o_nll, o_g, o_h)
+        e2e_step()
     barrier()
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        pwa.pwa_nll_grad_hvp_host(m.h, th_h, v_h, o_nll, o_g, o_h)
+        e2e_step()
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
+    if sharded_e2e and world == 1:
+        assert abs(float(pin_out[0]) - nll_dev) <= 1e-12 * abs(nll_dev), "sharded e2e path disagrees with the fused call"
     if world > 1:
         t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
