@@ -40,7 +40,7 @@ struct pwa_handle {
   pwa::LaneArgs largs;
   size_t lanes_smem = 0;
   int lanes_combo = -1;
-  int lanes_combo_alt = -1, block_alt = 0;  // shape of the gradient modes (MODE_GRAD, MODE_GRAD3), if another one
+  int lanes_combo_alt = -1, block_alt = 0;  // shape of the lighter modes (MODE_GRAD, MODE_GRAD3, MODE_HVPQ), if another one
   bool weight_padded = false;  // the data weights are library-owned and padded to an even length
 
   // device staging for the *_host entry point and the fit driver
@@ -67,7 +67,7 @@ typedef void (*lanes_fn)(const LaneArgs);
 struct LanesCombo {
   int rho, log_sw, nw, prod, tile, alt;  // resonances per lane, log2(slices per warp), compute warps per block, producer kind
                                     // (0 warp, 2 warpgroup), events per tile (32, or 8 with the swizzled layout), and the
-                                    // entry (same rho, slices, tile) used for the gradient modes, whose registers allow a
+                                    // entry (same rho, slices, tile) used for the modes with fewer accumulators, whose registers allow a
                                     // third compute warp per scheduler (-1: none)
 };
 // instantiated shapes (pwa_sweep_lanes_inst.cu); capacity RHO << LOG_SW resonances; the handle takes the first entry of

@@ -133,7 +133,7 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
   const size_t smem = (size_t)stages * stage_bytes + fixed;
 
   for (int mode = 0; mode < 5; ++mode) {
-    const bool use_alt = kLanesCombos[combo].alt >= 0 && (mode == MODE_GRAD || mode == MODE_GRAD3);
+    const bool use_alt = kLanesCombos[combo].alt >= 0 && (mode == MODE_GRAD || mode == MODE_GRAD3 || mode == MODE_HVPQ);
     const int cmb = use_alt ? kLanesCombos[combo].alt : combo;
     const int nthr = lanes::lanes_threads(kLanesCombos[cmb].nw, kLanesCombos[cmb].prod);
     lanes_fn fn = lanes_kernel(H, cmb, mode);
@@ -195,7 +195,7 @@ pwa_status lanes_launch(pwa_handle* h, int mode, const double* theta, const doub
   a.theta = theta;
   a.v = v;
   a.partial = h->d_partial;
-  const bool use_alt = h->lanes_combo_alt >= 0 && (mode == MODE_GRAD || mode == MODE_GRAD3);
+  const bool use_alt = h->lanes_combo_alt >= 0 && (mode == MODE_GRAD || mode == MODE_GRAD3 || mode == MODE_HVPQ);
   lanes_fn fn = lanes_kernel(h->n_hel, use_alt ? h->lanes_combo_alt : h->lanes_combo, mode);
   fn<<<h->grid, use_alt ? h->block_alt : h->block, h->lanes_smem, h->stream>>>(a);
   if (cudaError_t ce = cudaGetLastError()) return set_error(h, PWA_ERR_CUDA, "launch lanes sweep kernel", ce);
