@@ -21,6 +21,7 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--bursts", type=int, default=6)
+    ap.add_argument("--long", type=int, default=0, help="instead: N fused sweeps back to back, mean time per block of 25")
     args = ap.parse_args()
     import torch
     import paper_2403_09225_b200 as pwa
@@ -36,6 +37,25 @@ def main():
     if os.path.exists(pk):
         peak = float(json.load(open(pk))["hbm_gbs"])
     nbytes = pwa.pwa_bytes_per_eval(m.h)
+    if args.long > 0:
+        # the SM clock sags under this FP64 load after some tens of milliseconds: show the time per step along a long run
+        torch.cuda.synchronize()
+        time.sleep(2.0)
+        n = args.long
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(n + 1)]
+        ev[0].record()
+        for i in range(n):
+            pwa.pwa_nll_grad_hvp(m.h, th, v, m.nll_t, m.grad_t, m.hv_t)
+            ev[i + 1].record()
+        torch.cuda.synchronize()
+        ts = [ev[i].elapsed_time(ev[i + 1]) for i in range(n)]
+        print(f"config {args.config}: {pwa.pwa_kernel_variant(m.h)}; {n} fused sweeps back to back after a 2 s pause")
+        print("| steps | mean ms per step | fraction of the HBM peak |\n|---|---|---|")
+        for a in range(0, n, 25):
+            blk = ts[a:a + 25]
+            ms = sum(blk) / len(blk)
+            print(f"| {a}-{a + len(blk) - 1} | {ms:.4f} | {nbytes / ms / 1e6 / peak:.3f} |")
+        return
     calls = [("pwa_nll", lambda: pwa.pwa_nll(m.h, th, m.nll_t)),
              ("pwa_nll_grad", lambda: pwa.pwa_nll_grad(m.h, th, m.nll_t, m.grad_t)),
              ("pwa_nll_grad_for_hvp", lambda: pwa.pwa_nll_grad_for_hvp(m.h, th, m.nll_t, m.grad_t)),
