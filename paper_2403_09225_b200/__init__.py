@@ -309,61 +309,75 @@ def pwa_version() -> str:
 
 # ---- a small convenience wrapper (still marshalling only) ---------------------------------------------------
 class Model:
-    """Owns a handle and its output tensors.  `w` is a workloads.Workload (or any object with the same fields)."""
+    """Owns a handle and its output tensors.  `w` is a workloads.Workload (or any object with the same fields).
+    With `stream` (a cudaStream_t) the handle enqueues there, and so does every torch operation of this class."""
 
-    def __init__(self, w, device: int = 0, borrow: bool = False):
+    def __init__(self, w, device: int = 0, borrow: bool = False, stream: int = 0):
+        import contextlib
         import torch
         self.torch = torch
         self.dev = torch.device("cuda", device)
         self._keep = w if borrow else None
+        self._ext = torch.cuda.ExternalStream(stream, device=self.dev) if stream else None
+        self._on = (lambda: torch.cuda.stream(self._ext)) if stream else contextlib.nullcontext
         self.h = pwa_create(w.res_chan, w.data_mass, w.data_amp, w.data_weight, w.mc_mass, w.mc_amp, borrow=borrow,
-                            device=device)
+                            device=device, stream=stream)
         self.P = pwa_n_params(self.h)
-        self.nll_t = torch.zeros(1, dtype=torch.float64, device=self.dev)
-        self.grad_t = torch.zeros(self.P, dtype=torch.float64, device=self.dev)
-        self.hv_t = torch.zeros(self.P, dtype=torch.float64, device=self.dev)
+        with self._on():
+            self.nll_t = torch.zeros(1, dtype=torch.float64, device=self.dev)
+            self.grad_t = torch.zeros(self.P, dtype=torch.float64, device=self.dev)
+            self.hv_t = torch.zeros(self.P, dtype=torch.float64, device=self.dev)
 
     def _d(self, x):
         return self.torch.as_tensor(x, dtype=self.torch.float64).to(self.dev).contiguous()
 
     def nll(self, theta):
-        pwa_nll(self.h, self._d(theta), self.nll_t)
-        return self.nll_t.item()
+        with self._on():
+            pwa_nll(self.h, self._d(theta), self.nll_t)
+            return self.nll_t.item()
 
     def nll_grad(self, theta):
-        pwa_nll_grad(self.h, self._d(theta), self.nll_t, self.grad_t)
-        return self.nll_t.item(), self.grad_t.cpu().numpy().copy()
+        with self._on():
+            pwa_nll_grad(self.h, self._d(theta), self.nll_t, self.grad_t)
+            return self.nll_t.item(), self.grad_t.cpu().numpy().copy()
 
     def hvp(self, theta, v):
-        pwa_hvp(self.h, self._d(theta), self._d(v), self.hv_t)
-        return self.hv_t.cpu().numpy().copy()
+        with self._on():
+            pwa_hvp(self.h, self._d(theta), self._d(v), self.hv_t)
+            return self.hv_t.cpu().numpy().copy()
 
     def nll_grad_hvp(self, theta, v):
-        pwa_nll_grad_hvp(self.h, self._d(theta), self._d(v), self.nll_t, self.grad_t, self.hv_t)
-        return self.nll_t.item(), self.grad_t.cpu().numpy().copy(), self.hv_t.cpu().numpy().copy()
+        with self._on():
+            pwa_nll_grad_hvp(self.h, self._d(theta), self._d(v), self.nll_t, self.grad_t, self.hv_t)
+            return self.nll_t.item(), self.grad_t.cpu().numpy().copy(), self.hv_t.cpu().numpy().copy()
 
     def raw_sums(self, theta, v=None):
-        raw = self.torch.zeros(4 + 4 * self.P, dtype=self.torch.float64, device=self.dev)
-        pwa_raw_sums(self.h, self._d(theta), None if v is None else self._d(v), raw)
-        return raw
+        with self._on():
+            raw = self.torch.zeros(4 + 4 * self.P, dtype=self.torch.float64, device=self.dev)
+            pwa_raw_sums(self.h, self._d(theta), None if v is None else self._d(v), raw)
+            return raw
 
     def nll_grad_for_hvp(self, theta):
-        pwa_nll_grad_for_hvp(self.h, self._d(theta), self.nll_t, self.grad_t)
-        return self.nll_t.item(), self.grad_t.cpu().numpy().copy()
+        with self._on():
+            pwa_nll_grad_for_hvp(self.h, self._d(theta), self.nll_t, self.grad_t)
+            return self.nll_t.item(), self.grad_t.cpu().numpy().copy()
 
     def hvp_cached(self, v):
-        pwa_hvp_cached(self.h, self._d(v), self.hv_t)
-        return self.hv_t.cpu().numpy().copy()
+        with self._on():
+            pwa_hvp_cached(self.h, self._d(v), self.hv_t)
+            return self.hv_t.cpu().numpy().copy()
 
     def fit_fractions(self, theta):
-        frac = self.torch.zeros(self.P // 4, dtype=self.torch.float64, device=self.dev)
-        pwa_fit_fractions(self.h, self._d(theta), frac)
-        return frac.cpu().numpy()
+        with self._on():
+            frac = self.torch.zeros(self.P // 4, dtype=self.torch.float64, device=self.dev)
+            pwa_fit_fractions(self.h, self._d(theta), frac)
+            return frac.cpu().numpy()
 
     def fit(self, theta0, opts: Optional[pwa_fit_opts] = None):
-        th = self._d(theta0).clone()
-        res = pwa_fit_newton_cg(self.h, th, opts)
-        return th.cpu().numpy().copy(), res
+        with self._on():
+            th = self._d(theta0).clone()
+            res = pwa_fit_newton_cg(self.h, th, opts)
+            return th.cpu().numpy().copy(), res
 
     def close(self):
         if self.h:

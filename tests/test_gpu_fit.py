@@ -101,3 +101,27 @@ def test_wall_time_cap_stops_the_fit(setup):
     th, res = gm.fit(th0, _opts(pwa, max_seconds=1e-7))
     assert res.stop_reason == 5 and res.status == 5 and res.outer_iters <= 1
     assert np.isfinite(res.nll) and res.nll <= gm.nll(th0) + 1e-9 * abs(res.nll)
+
+
+def test_handles_on_their_own_streams_give_the_same_bits(setup):
+    """Two fits in flight on two handles and streams over the same event store (bench.py --concurrent) must reproduce,
+    bit for bit, what one handle on the default stream gives: nothing is shared between handles."""
+    import concurrent.futures as cf
+    pwa, workloads, models = setup
+    cfg, w, om, gm = models[2]
+    wd = type(w)(**{k: (v.cuda() if isinstance(v, torch.Tensor) and k != "res_chan" and k != "theta_true" else v)
+                    for k, v in w.__dict__.items()})
+    streams = [torch.cuda.Stream() for _ in range(2)]
+    hs = [pwa.Model(wd, borrow=True, stream=s.cuda_stream) for s in streams]
+    ref = pwa.Model(wd, borrow=True)
+    try:
+        starts = [workloads.random_start(cfg, k).numpy() for k in range(4)]
+        o = _opts(pwa, max_outer=8)
+        want = [ref.fit(s, o) for s in starts]
+        with cf.ThreadPoolExecutor(max_workers=2) as ex:
+            got = list(ex.map(lambda k: hs[k % 2].fit(starts[k], o), range(4)))
+        for (th0, r0), (th1, r1) in zip(want, got):
+            assert th0.tobytes() == th1.tobytes() and r0.nll == r1.nll and r0.n_hvp == r1.n_hvp
+    finally:
+        for x in hs + [ref]:
+            x.close()
