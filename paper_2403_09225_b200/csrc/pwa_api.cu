@@ -72,7 +72,8 @@ static size_t generic_smem(int block, int nb) { return (size_t)(block / 32) * ((
 
 // Runs prologue + sweep + stage-2 reduction/unpack; leaves the public raw vector in `raw` (device).
 static pwa_status raw_sums_impl(pwa_handle* h, int mode, const double* theta, const double* v, double* raw,
-                                bool combine = false, double* nll = nullptr, double* grad = nullptr, double* hv = nullptr) {
+                                bool combine = false, double* nll = nullptr, double* grad = nullptr, double* hv = nullptr,
+                                const double* skip = nullptr) {
   const int R = h->n_res;
   if (mode == MODE_FULL && !v) mode = MODE_GRAD;
   const bool prof = h->profiling && h->prof_used + 2 <= h->prof_events.size();
@@ -81,7 +82,7 @@ static pwa_status raw_sums_impl(pwa_handle* h, int mode, const double* theta, co
   if (packed) {
     // lanes sweep: the per-resonance constants are formed by every block itself (no prologue launch)
     if (prof) cudaEventRecord(h->prof_events[h->prof_used], h->stream);
-    pwa_status st = lanes_launch(h, mode, theta, mode_q(mode) ? v : nullptr);
+    pwa_status st = lanes_launch(h, mode, theta, mode_q(mode) ? v : nullptr, skip);
     if (st != PWA_OK) return st;
     h->launches++;
     if (prof) {
@@ -115,7 +116,7 @@ static pwa_status raw_sums_impl(pwa_handle* h, int mode, const double* theta, co
 #define PWA_REDUCE(M)                                                                                              \
   k_reduce_unpack<M><<<kReduceBlocks, 1024, 0, h->stream>>>(h->d_partial, h->grid, nb, R, packed, theta, v, n_mc,  \
                                                              h->d_sums, raw, combine ? 1 : 0, nll, grad, hv,        \
-                                                             h->d_flags, h->d_flags + 1, h->d_pcache)
+                                                             h->d_flags, h->d_flags + 1, h->d_pcache, skip)
   switch (mode) {
     case MODE_NLL: PWA_REDUCE(MODE_NLL); break;
     case MODE_GRAD: PWA_REDUCE(MODE_GRAD); break;
@@ -152,10 +153,10 @@ pwa_status eval_grad_keep(pwa_handle* h, const double* theta, double* nll, doubl
   return raw_sums_impl(h, MODE_GRAD3, h->d_theta_keep, nullptr, h->d_raw, true, nll, grad, nullptr);
 }
 
-pwa_status eval_hvp_kept(pwa_handle* h, const double* v, double* hv) {
+pwa_status eval_hvp_kept(pwa_handle* h, const double* v, double* hv, const double* skip) {
   if (!h->keep_valid) return set_error(h, PWA_ERR_INVALID_ARG, "pwa_hvp_cached: no pwa_nll_grad_for_hvp call before", cudaSuccess);
   if (h->variant < 2) return eval(h, MODE_FULL, h->d_theta_keep, v, nullptr, nullptr, hv);
-  return raw_sums_impl(h, MODE_HVPQ, h->d_theta_keep, v, h->d_raw, true, nullptr, nullptr, hv);
+  return raw_sums_impl(h, MODE_HVPQ, h->d_theta_keep, v, h->d_raw, true, nullptr, nullptr, hv, skip);
 }
 
 }  // namespace pwa

@@ -60,6 +60,7 @@ __global__ void __launch_bounds__(FT) k_cg_start(int P, const double* g, double*
     sc[S_GINF] = isfinite(ss) ? mx : CUDART_NAN;
     sc[S_GNORM] = gn;
     sc[S_EPS] = fmin(0.5, sqrt(gn)) * gn;
+    sc[S_STATUS] = 0.0;  // CG running (the speculative launches of the driver test this slot)
   }
 }
 
@@ -68,6 +69,7 @@ __global__ void __launch_bounds__(FT) k_cg_start(int P, const double* g, double*
 __global__ void __launch_bounds__(FT) k_cg_iter(int P, int j, const double* g, const double* q, double* z, double* r,
                                                 double* d, double* p, double* sc) {
   __shared__ double red[FT];
+  if (sc[S_STATUS] != 0.0) return;  // CG already ended: this iteration was enqueued speculatively
   double dq = 0.0, dd = 0.0;
   for (int k = threadIdx.x; k < P; k += FT) {
     dq = fma(d[k], q[k], dq);
@@ -171,6 +173,13 @@ extern "C" pwa_status pwa_fit_newton_cg(pwa_handle* h, double* theta, const pwa_
   const auto t0 = std::chrono::steady_clock::now();
   auto elapsed = [&] { return std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count(); };
   *res = pwa_fit_result{};
+  struct Events {
+    cudaEvent_t e[2] = {nullptr, nullptr};
+    ~Events() { for (cudaEvent_t x : e) if (x) cudaEventDestroy(x); }
+    cudaEvent_t& operator[](int i) { return e[i]; }
+  } ev;
+  for (int i = 0; i < 2; ++i)
+    if (cudaError_t ce = cudaEventCreateWithFlags(&ev[i], cudaEventDisableTiming)) return pwa::set_error(h, PWA_ERR_CUDA, "cudaEventCreate", ce);
   const int P = h->n_par;
   cudaStream_t st = h->stream;
   double *g = h->d_fit, *z = g + P, *r = z + P, *d = r + P, *q = d + P, *p = q + P, *trial = p + P, *sc = trial + P;
@@ -210,17 +219,37 @@ extern "C" pwa_status pwa_fit_newton_cg(pwa_handle* h, double* theta, const pwa_
     if (o.max_seconds > 0.0 && elapsed() > o.max_seconds) { stop = 5; break; }
     res->outer_iters = outer + 1;
 
-    // step 3: truncated CG on H p = -g
+    // step 3: truncated CG on H p = -g.  Iteration j + 1 is enqueued BEFORE the host has seen the verdict of iteration
+    // j (a copy of the status slot into pinned memory + an event per iteration): its kernels test the device-side
+    // status and return at once if CG has ended, so the host round trip hides behind the next sweep.  Shapes on the
+    // generic kernel have no such test and run one iteration at a time.
     bool have_p = false;
+    const bool pipelined = h->variant >= 2;
+    int done_at = -1;
     for (int j = 0; j < o.max_cg; ++j) {
-      FIT_EVAL(pwa::eval_hvp_kept(h, d, q));
-      res->n_hvp++;
-      res->cg_iters++;
+      FIT_EVAL(pwa::eval_hvp_kept(h, d, q, pipelined ? sc + S_STATUS : nullptr));
       k_cg_iter<<<1, FT, 0, st>>>(P, j, g, q, z, r, d, p, sc);
       h->launches++;
-      FIT_CHECK(fetch());
-      if (hs[S_STATUS] != 0.0) { have_p = true; break; }
+      if (!pipelined) {
+        FIT_CHECK(fetch());
+        if (hs[S_STATUS] != 0.0) { done_at = j; break; }
+        continue;
+      }
+      FIT_CHECK(cudaMemcpyAsync(hs + S_N + (j & 1), sc + S_STATUS, sizeof(double), cudaMemcpyDeviceToHost, st));
+      FIT_CHECK(cudaEventRecord(ev[j & 1], st));
+      if (j >= 1) {
+        FIT_CHECK(cudaEventSynchronize(ev[(j - 1) & 1]));
+        if (hs[S_N + ((j - 1) & 1)] != 0.0) { done_at = j - 1; break; }
+      }
+      if (j == o.max_cg - 1) {
+        FIT_CHECK(cudaEventSynchronize(ev[j & 1]));
+        if (hs[S_N + (j & 1)] != 0.0) done_at = j;
+      }
     }
+    have_p = done_at >= 0;
+    const int iters = have_p ? done_at + 1 : o.max_cg;
+    res->n_hvp += iters;
+    res->cg_iters += iters;
     if (!have_p) {
       k_copy<<<1, FT, 0, st>>>(P, z, p);
       h->launches++;

@@ -83,12 +83,12 @@ lanes_fn lanes_kernel_h3(int combo, int mode);
 lanes_fn lanes_kernel_h4(int combo, int mode);
 lanes_fn lanes_kernel(int H, int combo, int mode);
 pwa_status lanes_configure(pwa_handle* h, std::string& why);  // sets variant = 2 on success; PWA_OK + why if unsuitable
-pwa_status lanes_launch(pwa_handle* h, int mode, const double* theta, const double* v);
+pwa_status lanes_launch(pwa_handle* h, int mode, const double* theta, const double* v, const double* skip = nullptr);
 // internal entry points used by the fit driver (enqueue only)
 pwa_status eval(pwa_handle* h, int mode, const double* theta, const double* v, double* nll, double* grad,
                 double* hv);
 pwa_status eval_grad_keep(pwa_handle* h, const double* theta, double* nll, double* grad);
-pwa_status eval_hvp_kept(pwa_handle* h, const double* v, double* hv);
+pwa_status eval_hvp_kept(pwa_handle* h, const double* v, double* hv, const double* skip = nullptr);  // skip: LaneArgs::skip
 pwa_status set_error(pwa_handle* h, pwa_status st, const char* what, cudaError_t ce);
 }  // namespace pwa
 

@@ -358,7 +358,8 @@ __global__ void __launch_bounds__(1024) k_reduce_unpack(const double* __restrict
                                                         const double* __restrict__ v, double n_mc, double* sums, double* raw,
                                                         int combine, double* __restrict__ nll, double* __restrict__ grad,
                                                         double* __restrict__ hv, unsigned* __restrict__ flags,
-                                                        unsigned* ticket, double* pcache) {
+                                                        unsigned* ticket, double* pcache, const double* skip) {
+  if (skip != nullptr && *skip != 0.0) return;  // see LaneArgs::skip
   constexpr int VPR = vpr_of(MODE), RPB = rpb_of(MODE);
   const int nacc = packed ? (MODE == MODE_NLL ? 0 : R * VPR) : nb * 32, stride = nacc + 2, P = 4 * R;
   // Phase 1 over all blocks of this launch: block g sums the columns k = g * 1024 + t, (g + gridDim) * 1024 + t, ...

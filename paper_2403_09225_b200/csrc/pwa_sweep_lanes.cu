@@ -190,10 +190,11 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
   return PWA_OK;
 }
 
-pwa_status lanes_launch(pwa_handle* h, int mode, const double* theta, const double* v) {
+pwa_status lanes_launch(pwa_handle* h, int mode, const double* theta, const double* v, const double* skip) {
   LaneArgs a = h->largs;
   a.theta = theta;
   a.v = v;
+  a.skip = skip;
   a.partial = h->d_partial;
   const bool use_alt = h->lanes_combo_alt >= 0 && (mode == MODE_GRAD || mode == MODE_GRAD3 || mode == MODE_HVPQ);
   lanes_fn fn = lanes_kernel(h->n_hel, use_alt ? h->lanes_combo_alt : h->lanes_combo, mode);

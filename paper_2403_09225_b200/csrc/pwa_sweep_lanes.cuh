@@ -34,6 +34,8 @@ struct alignas(64) LaneArgs {
   int weighted;  // data events carry weights
   const double* theta;
   const double* v;
+  const double* skip;  // optional device scalar: a non-zero value turns this launch into a no-op (speculative CG
+                       // iterations of the fit driver enqueued before the previous iteration's verdict is known)
   const int* ch;
   double* partial;  // [2][gridDim.x][R*NACC + 2]
   int R, C, stages;
@@ -249,6 +251,7 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
   constexpr int NA = NACC > 0 ? NACC : 1;
   constexpr int RP = RHO * SW;             // resonances incl. padding
   extern __shared__ __align__(1024) unsigned char smem_raw[];
+  if (a.skip != nullptr && *a.skip != 0.0) return;  // uniform over the grid
   const int lane = threadIdx.x & 31, w = (int)(threadIdx.x >> 5) - (PROD == 2 ? 4 : 0);  // w: compute-warp index
   const int R = a.R, stages = a.stages;
   double* Ks = reinterpret_cast<double*>(smem_raw + a.off_K);    // [RP][KS]
