@@ -350,7 +350,10 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
   }
   double* xrow = reinterpret_cast<double*>(smem_raw + a.off_xch) + ((size_t)w * EW + e) * (4 * H);  // this event's exchange row
 
-  // pass g = w + k NW  ->  local tile t = g / NP, column col = g % NP
+  // pass g = w + k NW  ->  local tile t = g / NP, column col = g % NP.  When NW is a multiple of NP a warp keeps
+  // its column for the whole sweep (FIXCOL): the event index, the amplitude and mass offsets inside a stage are then
+  // loop constants and a pass only adds the stage base.
+  constexpr bool FIXCOL = NW % NP == 0;
   int t = w / NP, col = w % NP;
   int st = t % stages, ph = (t / stages) & 1;
 
@@ -542,13 +545,24 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
       }
 
       // ---------------- next pass of this warp ----------------
-      col += NW;
-      while (col >= NP) {
-        col -= NP;
-        ++t;
-        if (++st == stages) {
-          st = 0;
-          ph ^= 1;
+      if (FIXCOL) {
+#pragma unroll
+        for (int k = 0; k < NW / NP; ++k) {
+          ++t;
+          if (++st == stages) {
+            st = 0;
+            ph ^= 1;
+          }
+        }
+      } else {
+        col += NW;
+        while (col >= NP) {
+          col -= NP;
+          ++t;
+          if (++st == stages) {
+            st = 0;
+            ph ^= 1;
+          }
         }
       }
     }
