@@ -68,12 +68,13 @@ struct LanesCombo {
   int rho, log_sw, nw, prod, tile, alt;  // resonances per lane, log2(slices per warp), compute warps per block, producer kind
                                     // (0 warp, 2 warpgroup), events per tile (32, or 8 with the swizzled layout), and the
                                     // entry (same rho, slices, tile) used for the modes with fewer accumulators, whose registers allow a
-                                    // third compute warp per scheduler (-1: none)
+                                    // third compute warp per scheduler (-1: none; no entry uses one since warps keep their columns:
+                                    // the 8-warp warpgroup shape then measured faster in every mode)
 };
 // instantiated shapes (pwa_sweep_lanes_inst.cu); capacity RHO << LOG_SW resonances; the handle takes the first entry of
 // the smallest capacity >= R whose stages fit in shared memory at least twice
 constexpr LanesCombo kLanesCombos[] = {
-    {1, 2, 15, 0, 32, -1}, {2, 3, 15, 0, 32, -1}, {3, 2, 11, 0, 32, -1}, {3, 2, 8, 2, 32, -1}, {4, 3, 8, 2, 32, 12}, {4, 3, 7, 0, 32, -1},
+    {1, 2, 15, 0, 32, -1}, {2, 3, 15, 0, 32, -1}, {3, 2, 11, 0, 32, -1}, {3, 2, 8, 2, 32, -1}, {4, 3, 8, 2, 32, -1}, {4, 3, 7, 0, 32, -1},
     {4, 4, 8, 2, 32, -1},  {4, 4, 7, 0, 32, -1},  {4, 5, 8, 2, 32, -1},  {4, 5, 7, 0, 32, -1}, {4, 4, 8, 2, 8, -1},  {4, 5, 8, 2, 8, -1},
     {4, 3, 11, 3, 32, -1}};
 constexpr int kNumLanesCombos = sizeof(kLanesCombos) / sizeof(kLanesCombos[0]);

@@ -132,9 +132,10 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
   why.clear();
   const size_t smem = (size_t)stages * stage_bytes + fixed;
 
+  const int alt = kLanesCombos[combo].alt;
   for (int mode = 0; mode < 5; ++mode) {
-    const bool use_alt = kLanesCombos[combo].alt >= 0 && (mode == MODE_GRAD || mode == MODE_GRAD3 || mode == MODE_HVPQ);
-    const int cmb = use_alt ? kLanesCombos[combo].alt : combo;
+    const bool use_alt = alt >= 0 && (mode == MODE_GRAD || mode == MODE_GRAD3 || mode == MODE_HVPQ);
+    const int cmb = use_alt ? alt : combo;
     const int nthr = lanes::lanes_threads(kLanesCombos[cmb].nw, kLanesCombos[cmb].prod);
     lanes_fn fn = lanes_kernel(H, cmb, mode);
     cudaError_t ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, dev_smem);
@@ -180,7 +181,7 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
   a.off_bar = a.off_xch + xch_bytes;
   h->lanes_smem = smem;
   h->lanes_combo = combo;
-  h->lanes_combo_alt = kLanesCombos[combo].alt;
+  h->lanes_combo_alt = alt;
   if (h->lanes_combo_alt >= 0)
     h->block_alt = lanes::lanes_threads(kLanesCombos[h->lanes_combo_alt].nw, kLanesCombos[h->lanes_combo_alt].prod);
   h->variant = 2;
