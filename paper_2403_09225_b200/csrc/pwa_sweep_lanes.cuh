@@ -64,6 +64,17 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+// arrive by the lanes for which `who` is zero, as ONE predicated instruction (no divergent branch around it)
+__device__ __forceinline__ void mbar_arrive_if_zero(uint32_t bar, uint32_t who) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "setp.eq.u32 p, %1, 0;\n"
+      "@p mbarrier.arrive.shared::cta.b64 _, [%0];\n"
+      "}\n" ::"r"(bar),
+      "r"(who)
+      : "memory");
+}
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   asm volatile(
       "{\n"
@@ -447,7 +458,7 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
       }
       // everything this pass needs from the stage is in registers: hand the column back to the producer
       __syncwarp();
-      if (lane == 0) mbar_arrive(empty0 + 8 * st);
+      mbar_arrive_if_zero(empty0 + 8 * st, (uint32_t)lane);
 
       // ---------------- exchange over the slices ----------------
       slice_reduce_store<NV, EW>(x, lane, xrow);
