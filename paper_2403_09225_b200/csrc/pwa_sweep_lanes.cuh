@@ -348,8 +348,17 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
   // with the producer warpgroup the compute warps own 240 registers: keep the constants every pass needs in
   // registers instead of re-reading them from shared memory (one wavefront per 4 bytes per lane, broadcast or not)
   constexpr bool KREG = PROD == 2 && RHO * H <= 9;  // beyond that the amplitudes G_rh themselves fill the file
-  double2 creg[RHO], k01reg[RHO];
+  // MODE_HVPQ holds 24 fewer accumulators per lane than the fused mode: alpha, beta live in registers there too
+  // (in the fused mode the same change measured 4 % slower: no room)
+  constexpr int KAB = (KREG && MODE == MODE_HVPQ) ? RHO : 0;
+  double2 creg[RHO], k01reg[RHO], alreg[KAB > 0 ? KAB : 1], bereg[KAB > 0 ? KAB : 1];
   double mgreg[RHO];
+#pragma unroll
+  for (int j = 0; j < KAB; ++j) {
+    const double2* kk = reinterpret_cast<const double2*>(lane_k + j * (SW * KS));
+    alreg[j] = kk[3];
+    bereg[j] = kk[4];
+  }
   if (KREG) {
 #pragma unroll
     for (int j = 0; j < RHO; ++j) {
@@ -429,7 +438,7 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
         } else {
           double wr = 0.0, wi = 0.0;
           if (WQ) {  // zdot = (alpha + beta B) B
-            const double2 al = kk[3], be = kk[4];
+            const double2 al = j < KAB ? alreg[j < KAB ? j : 0] : kk[3], be = j < KAB ? bereg[j < KAB ? j : 0] : kk[4];
             wr = fma(be.x, br, fma(-be.y, bi, al.x));
             wi = fma(be.x, bi, fma(be.y, br, al.y));
           }
