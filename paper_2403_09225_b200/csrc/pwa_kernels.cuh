@@ -362,25 +362,22 @@ __global__ void __launch_bounds__(1024) k_reduce_unpack(const double* __restrict
   if (skip != nullptr && *skip != 0.0) return;  // see LaneArgs::skip
   constexpr int VPR = vpr_of(MODE), RPB = rpb_of(MODE);
   const int nacc = packed ? (MODE == MODE_NLL ? 0 : R * VPR) : nb * 32, stride = nacc + 2, P = 4 * R;
-  // Phase 1 over all blocks of this launch: block g sums the columns k = g * 1024 + t, (g + gridDim) * 1024 + t, ...
-  // (one SM cannot pull the 148 partial rows fast enough on its own).  The value of every column is independent of
-  // the block that computes it.
-  for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < 2 * stride; k += gridDim.x * blockDim.x) {
-    const int sample = k / stride, idx = k - sample * stride;
-    const double* p = partial + (size_t)sample * nblocks * stride + idx;
-    // four interleaved running sums (rows b = 0, 4, 8, ... / 1, 5, ... / ...) keep four loads in flight; the order of
-    // additions is fixed: ((t0 + t1) + (t2 + t3))
-    double t0 = 0.0, t1 = 0.0, t2 = 0.0, t3 = 0.0;
-    int b = 0;
-#pragma unroll 2
-    for (; b + 4 <= nblocks; b += 4) {
-      t0 += p[(size_t)b * stride];
-      t1 += p[(size_t)(b + 1) * stride];
-      t2 += p[(size_t)(b + 2) * stride];
-      t3 += p[(size_t)(b + 3) * stride];
+  // Phase 1 over all blocks of this launch: one WARP per column (warp W of the launch takes columns W, W + #warps, ...):
+  // lane l adds the rows l, l + 32, ... of the per-block partials in order, then a fixed butterfly over the lanes.  A
+  // thread per column would walk the 148 rows one L2 latency after the other; this way a column costs about five
+  // loads in flight and five shuffles.  The value of a column does not depend on the block that computes it.
+  {
+    const int lane = threadIdx.x & 31;
+    const int warps = (gridDim.x * blockDim.x) >> 5, wid = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    for (int k = wid; k < 2 * stride; k += warps) {
+      const int sample = k / stride, idx = k - sample * stride;
+      const double* p = partial + (size_t)sample * nblocks * stride + idx;
+      double t = 0.0;
+      for (int b = lane; b < nblocks; b += 32) t += p[(size_t)b * stride];
+#pragma unroll
+      for (int m = 16; m > 0; m >>= 1) t += __shfl_xor_sync(0xffffffffu, t, m);
+      if (lane == 0) sums[k] = t;
     }
-    for (; b < nblocks; ++b) t0 += p[(size_t)b * stride];
-    sums[k] = (t0 + t1) + (t2 + t3);
   }
   // The block that finishes last (whichever it is: the sums do not depend on it) unpacks and combines.
   if (gridDim.x > 1) {
