@@ -3,6 +3,8 @@
 // per CG iteration / line-search trial for control flow.
 #include <chrono>
 #include <cmath>
+#include <cstdio>
+#include <cstdlib>
 
 #include <math_constants.h>
 
@@ -170,6 +172,7 @@ extern "C" pwa_status pwa_fit_newton_cg(pwa_handle* h, double* theta, const pwa_
   if (opts_in) o = *opts_in; else pwa_fit_opts_default(&o);
   if (o.max_outer < 0 || o.max_cg < 1 || o.max_backtrack < 0 || !(o.backtrack > 0.0 && o.backtrack < 1.0))
     return pwa::set_error(h, PWA_ERR_INVALID_ARG, "pwa_fit_newton_cg: bad options", cudaSuccess);
+  const bool trace = std::getenv("PWA_FIT_TRACE") != nullptr;  // per-iteration diagnostics on stderr
   const auto t0 = std::chrono::steady_clock::now();
   auto elapsed = [&] { return std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count(); };
   *res = pwa_fit_result{};
@@ -261,6 +264,7 @@ extern "C" pwa_status pwa_fit_newton_cg(pwa_handle* h, double* theta, const pwa_
     double t = 1.0, fnew = 0.0;
     bool accepted = false;
     double gp = 0.0, pinf = 0.0;
+    int n_infeasible = 0;
     for (int bt = 0; bt <= o.max_backtrack; ++bt) {
       k_trial<<<1, FT, 0, st>>>(P, theta, p, t, trial, o.gamma_min, o.gamma_max, o.mass_min, o.mass_max, sc);
       h->launches++;
@@ -271,8 +275,12 @@ extern "C" pwa_status pwa_fit_newton_cg(pwa_handle* h, double* theta, const pwa_
       pinf = hs[S_PINF];
       fnew = hs[S_FTRIAL];
       if (hs[S_FEAS] != 0.0 && std::isfinite(fnew) && fnew <= f + o.armijo_c1 * t * gp) { accepted = true; break; }
+      if (hs[S_FEAS] == 0.0) ++n_infeasible;
       t *= o.backtrack;
     }
+    if (trace)
+      std::fprintf(stderr, "pwa_fit: outer %d f %.10e |g|inf %.3e cg %d (end %d) g.p %.3e |p|inf %.3e t %.3e infeasible %d f_new %.10e %s\n",
+                   outer, f, ginf, iters, have_p ? (int)hs[S_STATUS] : 0, gp, pinf, t, n_infeasible, fnew, accepted ? "ok" : "LINE SEARCH FAILED");
     if (!accepted) { stop = 6; break; }
     // step 5: accept
     FIT_CHECK(cudaMemcpyAsync(theta, trial, sizeof(double) * P, cudaMemcpyDeviceToDevice, st));

@@ -175,6 +175,34 @@ def test_p3_closed_form_bw_integral_uniform_in_s(oracle_mod):
     assert abs(got - want) < 2e-12 * want
 
 
+def test_p3_full_nll_closed_form_pins_the_additive_constant(oracle_mod):
+    """The WHOLE NLL of Eq. 3 (readings S2, S3) in closed form, additive constant included:
+    R = 1, H = 1, F = 1, MC masses on a midpoint grid uniform in s = m^2 over [lo^2, hi^2], five weighted data events
+    at chosen masses:
+        NLL = - sum_i w_i ln( a^2 / ((M^2 - m_i^2)^2 + M^2 Gamma^2) ) + W ln( a^2 J / (hi^2 - lo^2) ),
+        J = [atan((s - M^2)/(M Gamma))] over [lo^2, hi^2] / (M Gamma),    W = sum_i w_i,
+    evaluated here with numpy only.  Every other pin is blind to a theta-independent shift of the NLL (they differentiate
+    it or compare two NLLs that share W and N_mc); a dropped 1/N_mc inside the logarithm, or a logarithm of another
+    base, changes this value by W ln N_mc (= 65) or by a factor ln 10 and fails here."""
+    o = oracle_mod
+    lo, hi, N = 0.3, 3.0, 400_000
+    s = lo * lo + (np.arange(N) + 0.5) * (hi * hi - lo * lo) / N
+    amp = np.zeros((1, 1, N, 2)); amp[..., 0] = 1.0
+    mc = o.Sample(np.sqrt(s).reshape(1, N), amp, None)
+    md = np.array([0.45, 1.1, 1.31, 1.9, 2.7])
+    w = np.array([0.5, 1.5, 1.0, 0.75, 1.25])
+    ad = np.zeros((1, 1, md.size, 2)); ad[..., 0] = 1.0
+    m = o.Model(np.zeros(1, np.int32), o.Sample(md.reshape(1, -1), ad, w), mc)
+    a, phi, M, G = 1.7, 0.4, 1.3, 0.07
+    J = (np.arctan((hi * hi - M * M) / (M * G)) - np.arctan((lo * lo - M * M) / (M * G))) / (M * G)
+    want = -np.sum(w * np.log(a * a / ((M * M - md * md) ** 2 + (M * G) ** 2))) + w.sum() * np.log(a * a * J / (hi * hi - lo * lo))
+    for prec in ("ld", "d"):
+        got = float(o.nll(m, np.array([a, phi, M, G]), prec))
+        assert abs(got - want) < 1e-11 * abs(want), (prec, got, want)
+    # the constant really is visible to this test: the two plausible mistakes named above move the value far outside
+    assert abs(w.sum() * np.log(N)) > 1e3 * 1e-11 * abs(want) and abs(want) * (1 - 1 / np.log(10)) > 1.0
+
+
 # ----------------------------------------------------------------------------------------------- P4
 def test_p4_mc_term_is_a_hermitian_form_in_the_couplings(oracle_mod):
     o = oracle_mod
