@@ -1,20 +1,27 @@
-"""Reference fit: truncated line-search Newton-CG on top of the CPU oracle's NLL / gradient / HVP.
+"""Reference fit: projected, truncated line-search Newton-CG on top of the CPU oracle's NLL / gradient / HVP.
 
-TEST INFRASTRUCTURE, NOT THE PRODUCT (same rule as oracle/__init__.py).  It follows SURVEY.md §8(c-F)
-(S15, S19) step by step, in that order and notation; the paper only names SciPy's Newton-CG
- and the configuration asks for "<= 50 CG iterations per outer step, Armijo line search"
-(BASELINE.json configs[4]).  Plain numpy, one HVP per CG iteration, no shortcuts:
+TEST INFRASTRUCTURE, NOT THE PRODUCT (same rule as oracle/__init__.py).  It follows DESIGN.md reading S15' / S19
+step by step, in that order and notation.  The paper only names SciPy's Newton-CG, mentions
+undefined "constraint conditions" and the configuration asks for "<= 50 CG iterations per outer step,
+Armijo line search" (BASELINE.json configs[4]).  The box of S19 (Gamma_r in [gamma_min, gamma_max], M_r in
+[mass_min, mass_max]; a_r, phi_r free) is treated the textbook way for bound constraints (Bertsekas, projected
+Newton; Nocedal & Wright, Numerical Optimization, ch. 16.7 gradient projection + Alg. 7.1 for the inner CG):
+variables that sit on a bound with the gradient pushing outward are frozen for the inner solve, and trial points are
+projected onto the box instead of being rejected.  Plain numpy, one HVP per CG iteration, no shortcuts:
 
-  1. f, g at theta.  Stop (gtol) if |g|_inf <= gtol.
-  2. eps = min(0.5, sqrt(|g|_2)) |g|_2 ;  z = 0, r = g, d = -g.
-  3. for j < max_cg:  q = H d;  gamma = d.q.
-       if gamma <= 1e-14 d.d:  p = -g if j == 0 else z;  leave.
+  0. theta <- clip(theta0, lo, hi).
+  1. f, g at theta.  Active set A = {k : (theta_k <= lo_k and g_k > 0) or (theta_k >= hi_k and g_k < 0)};
+     projected gradient gP = g with the entries of A set to 0.  Stop (1) if |gP|_inf <= gtol.
+  2. eps = min(0.5, sqrt(|gP|_2)) |gP|_2 ;  z = 0, r = gP, d = -gP.
+  3. for j < max_cg:  q = H d with the entries of A set to 0;  gamma = d.q.
+       if gamma <= 1e-14 d.d:  p = -gP if j == 0 else z;  leave.
        alpha = r.r / gamma;  z += alpha d;  r_new = r + alpha q;  if |r_new|_2 <= eps:  p = z;  leave.
        beta = r_new.r_new / r.r;  d = -r_new + beta d;  r = r_new.            exhausted:  p = z.
-  4. Armijo: t = 1; while theta + t p leaves the box (S19), or f(theta + t p) is not finite, or
-       f(theta + t p) > f + c1 t g.p :  t *= rho;  give up after max_backtrack shrinks.
-  5. theta += t p.  Stop if t |p|_inf <= xtol (2) or |f_new - f| <= ftol max(1, |f|) (3), or max_outer (4).
-  converged  <=>  stopped on test 1, 2 or 3  and  |g|_inf <= gconv.
+  4. Projected Armijo: t = 1; trial = clip(theta + t p), s = trial - theta; while f(trial) is not finite or
+       f(trial) > f + c1 g.s :  t *= rho.  After max_backtrack shrinks: if p was not -gP, restart this step once with
+       p = -gP, t = 1; otherwise give up (6).
+  5. theta <- trial.  Stop if |s|_inf <= xtol (2) or |f_new - f| <= ftol max(1, |f|) (3), or max_outer (4).
+  converged  <=>  stopped on test 1, 2 or 3  and  |gP|_inf <= gconv  (gP of the final point).
 """
 from __future__ import annotations
 
@@ -55,23 +62,33 @@ class FitResult:
     n_hvp: int = 0
     stop_reason: int = 0
     converged: bool = False
+    n_active: int = 0
     trace: list = field(default_factory=list)
 
 
-def _feasible(theta: np.ndarray, o: FitOpts) -> bool:
-    M, G = theta[2::4], theta[3::4]
-    ok = True
-    if not (o.gamma_min == 0.0 and o.gamma_max == 0.0):
-        ok = ok and bool(np.all(G >= o.gamma_min) and np.all(G <= o.gamma_max))
+def bounds(n_par: int, o: FitOpts, dt=np.float64):
+    """lo[k], hi[k] of reading S19: only M (k % 4 == 2) and Gamma (k % 4 == 3) are boxed; a pair of zeros = no box."""
+    lo = np.full(n_par, -np.inf, dtype=dt)
+    hi = np.full(n_par, np.inf, dtype=dt)
     if not (o.mass_min == 0.0 and o.mass_max == 0.0):
-        ok = ok and bool(np.all(M >= o.mass_min) and np.all(M <= o.mass_max))
-    return ok
+        lo[2::4], hi[2::4] = o.mass_min, o.mass_max
+    if not (o.gamma_min == 0.0 and o.gamma_max == 0.0):
+        lo[3::4], hi[3::4] = o.gamma_min, o.gamma_max
+    return lo, hi
+
+
+def projected_gradient(theta, g, lo, hi):
+    """g with the entries of the active set (on a bound, gradient pushing outward) set to zero; the mask of free entries."""
+    active = ((theta <= lo) & (g > 0)) | ((theta >= hi) & (g < 0))
+    free = ~active
+    return np.where(free, g, 0), free
 
 
 def fit_newton_cg(model, theta0, opts: FitOpts | None = None, prec: str = "d", threads: int = 1) -> FitResult:
     o = opts or FitOpts()
     dt = np.longdouble if prec == "ld" else np.float64
-    theta = np.array(theta0, dtype=dt)
+    lo, hi = bounds(len(theta0), o, dt)
+    theta = np.clip(np.array(theta0, dtype=dt), lo, hi)  # step 0
     res = FitResult(theta=theta, nll=np.nan, grad_inf_norm=np.nan)
 
     def value_grad(th):
@@ -88,9 +105,11 @@ def fit_newton_cg(model, theta0, opts: FitOpts | None = None, prec: str = "d", t
     stop = 0
     outer = 0
     while True:
-        ginf = float(np.max(np.abs(g)))
+        # step 1
+        gP, free = projected_gradient(theta, g, lo, hi)
+        ginf = float(np.max(np.abs(gP)))
         res.trace.append((outer, float(f), ginf))
-        if not (np.isfinite(float(f)) and np.isfinite(ginf)):
+        if not (np.isfinite(float(f)) and np.isfinite(float(np.max(np.abs(g))))):
             stop = -1
             break
         if ginf <= o.gtol:
@@ -102,19 +121,19 @@ def fit_newton_cg(model, theta0, opts: FitOpts | None = None, prec: str = "d", t
         outer += 1
         res.outer_iters = outer
         # step 2
-        gnorm = float(np.sqrt(np.dot(g, g)))
+        gnorm = float(np.sqrt(np.dot(gP, gP)))
         eps = min(0.5, np.sqrt(gnorm)) * gnorm
-        z = np.zeros_like(g)
-        r = g.copy()
-        d = -g
+        z = np.zeros_like(gP)
+        r = gP.copy()
+        d = -gP
         p = None
         # step 3
         for j in range(o.max_cg):
-            q = hvp(theta, d)
+            q = np.where(free, hvp(theta, d), 0)
             res.cg_iters += 1
             gamma = np.dot(d, q)
-            if gamma <= 1e-14 * np.dot(d, d):
-                p = -g if j == 0 else z.copy()
+            if not (gamma > 1e-14 * np.dot(d, d)):
+                p = -gP if j == 0 else z.copy()
                 break
             rr = np.dot(r, r)
             alpha = rr / gamma
@@ -129,25 +148,29 @@ def fit_newton_cg(model, theta0, opts: FitOpts | None = None, prec: str = "d", t
         if p is None:
             p = z.copy()
         # step 4
-        gp = np.dot(g, p)
-        t = dt(1.0)
         accepted = False
         f_new = f
-        for _ in range(o.max_backtrack + 1):
-            trial = theta + t * p
-            if _feasible(trial, o):
+        is_sd = bool(np.array_equal(p, -gP))
+        while True:
+            t = dt(1.0)
+            for _ in range(o.max_backtrack + 1):
+                trial = np.clip(theta + t * p, lo, hi)
+                s = trial - theta
                 f_new = dt(_nll(model, trial, prec, threads=threads))
                 res.n_nll += 1
-                if np.isfinite(float(f_new)) and f_new <= f + o.armijo_c1 * t * gp:
+                if np.isfinite(float(f_new)) and f_new <= f + o.armijo_c1 * np.dot(g, s):
                     accepted = True
                     break
-            t = t * o.backtrack
+                t = t * o.backtrack
+            if accepted or is_sd:
+                break
+            p, is_sd = -gP, True  # one restart along the projected steepest descent
         if not accepted:
             stop = 6
             break
         # step 5
-        theta = theta + t * p
-        step_inf = float(t * np.max(np.abs(p)))
+        step_inf = float(np.max(np.abs(s)))
+        theta = trial
         f_old = f
         f, g = value_grad(theta)
         if step_inf <= o.xtol:
@@ -155,11 +178,14 @@ def fit_newton_cg(model, theta0, opts: FitOpts | None = None, prec: str = "d", t
         elif abs(float(f_new - f_old)) <= o.ftol * max(1.0, abs(float(f_old))):
             stop = 3
         if stop:
-            res.trace.append((outer, float(f), float(np.max(np.abs(g)))))
+            gP, free = projected_gradient(theta, g, lo, hi)
+            res.trace.append((outer, float(f), float(np.max(np.abs(gP)))))
             break
+    gP, free = projected_gradient(theta, g, lo, hi)
     res.theta = theta
     res.nll = float(f)
-    res.grad_inf_norm = float(np.max(np.abs(g)))
+    res.grad_inf_norm = float(np.max(np.abs(gP)))
+    res.n_active = int(np.sum(~free))
     res.stop_reason = stop
     res.converged = stop in (1, 2, 3) and res.grad_inf_norm <= o.gconv
     return res

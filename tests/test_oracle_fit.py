@@ -69,3 +69,46 @@ def test_box_is_respected_and_bad_start_is_reported(oracle_mod):
     assert np.all(th[2::4] >= o.mass_min) and np.all(th[2::4] <= o.mass_max)
     assert res.nll <= float(oracle_mod.nll(om, th0, "d"))
     assert res.stop_reason in (1, 2, 3, 4, 6)
+
+
+def test_active_bound_minimum_matches_scipy_lbfgsb(oracle_mod, toy):
+    """The projected Newton-CG of DESIGN.md S15'/S19 against SciPy's L-BFGS-B (an independent bound-constrained
+    optimiser) on a box that cuts the unconstrained minimum off: same NLL, KKT conditions at the returned point."""
+    from scipy.optimize import minimize
+    from oracle.fit import FitOpts, bounds, fit_newton_cg, projected_gradient
+    cfg, om, th0 = toy
+    free_fit = fit_newton_cg(om, th0, prec="d", threads=oracle_mod.max_threads())
+    g_hat = np.asarray(free_fit.theta, dtype=np.float64)[3::4]
+    # upper width bound below the smallest fitted width, lower mass bound above the smallest fitted mass
+    o = FitOpts(gamma_max=0.8 * float(g_hat.min()), mass_min=float(np.asarray(free_fit.theta, dtype=np.float64)[2::4].min()) + 0.02)
+    res = fit_newton_cg(om, th0, o, prec="d", threads=oracle_mod.max_threads())
+    assert res.converged and res.n_active >= 2 and res.nll > free_fit.nll
+    th = np.asarray(res.theta, dtype=np.float64)
+    lo, hi = bounds(len(th), o)
+    assert np.all(th >= lo) and np.all(th <= hi)
+    _, g, _ = oracle_mod.nll_grad_hvp(om, th, None, "d")
+    g = np.asarray(g, dtype=np.float64)
+    gP, free = projected_gradient(th, g, lo, hi)
+    assert float(np.max(np.abs(gP))) < 1e-2                 # stationary on the free variables
+    assert np.all(g[~free & (th <= lo)] > 0) and np.all(g[~free & (th >= hi)] < 0)  # multipliers have the right sign
+    vals = [f for (_, f, _) in res.trace]
+    assert all(b <= a + 1e-9 * abs(a) for a, b in zip(vals, vals[1:]))
+
+    fun = lambda t: float(oracle_mod.nll(om, t, "d"))
+    jac = lambda t: np.asarray(oracle_mod.nll_grad_hvp(om, t, None, "d")[1], dtype=np.float64)
+    sp = minimize(fun, np.clip(th0, lo, hi), jac=jac, method="L-BFGS-B", bounds=list(zip(lo, hi)),
+                  options={"maxiter": 2000, "ftol": 1e-15, "gtol": 1e-8})
+    assert abs(sp.fun - res.nll) <= 1e-7 * max(1.0, abs(sp.fun)), (sp.fun, res.nll)
+
+
+def test_start_outside_the_box_is_projected(oracle_mod):
+    from oracle.fit import FitOpts, fit_newton_cg
+    om = random_model(oracle_mod, 3, R=2, H=2, C=1, n_data=300, n_mc=1500, weighted=False)
+    th0 = random_theta(4, 2)
+    th0[3] = 5.0      # Gamma_0 above gamma_max
+    th0[6] = 0.01     # M_1 below mass_min
+    o = FitOpts(max_outer=0)
+    res = fit_newton_cg(om, th0, o, prec="d")
+    th = np.asarray(res.theta, dtype=np.float64)
+    assert th[3] == o.gamma_max and th[6] == o.mass_min and res.stop_reason == 4
+    assert res.nll == float(oracle_mod.nll(om, th, "d"))
