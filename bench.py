@@ -42,52 +42,128 @@ def _peaks():
 
 
 class ClockSampler:
-    """Samples nvidia-smi clocks and throttle reasons while the timed region runs."""
+    """Samples SM clock, power and throttle reasons while a timed region runs: NVML from a thread every ~2 ms
+    (so that samples fall inside regions of a few tens of milliseconds), nvidia-smi -lms 20 if NVML is unavailable."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
 
-    def __init__(self, index: int):
-        self.index, self.rows, self.proc, self.thread = index, [], None, None
+    def __init__(self, index: int, period_s: float = 0.002):
+        self.index, self.period, self.rows, self.proc, self.thread = index, period_s, [], None, None
+        self.stop_flag = threading.Event()
+        self.source = None
 
     def start(self):
         try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.dev = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_sm = float(pynvml.nvmlDeviceGetMaxClockInfo(self.dev, pynvml.NVML_CLOCK_SM))
+            self.source = "nvml"
+            self.thread = threading.Thread(target=self._poll_nvml, daemon=True)
+            self.thread.start()
+            return
+        except Exception:
+            self.source = None
+        try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.source = "nvidia-smi -lms 20"
         except OSError:
             self.proc = None
             return
-        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread = threading.Thread(target=self._read_smi, daemon=True)
         self.thread.start()
 
-    def _read(self):
-        for line in self.proc.stdout:
-            self.rows.append((time.time(), line.strip()))
-
-    def stop(self, t0: float, t1: float):
-        if self.proc is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
-        self.proc.terminate()
-        try:
-            self.proc.wait(timeout=2)
-        except Exception:
-            self.proc.kill()
-        inside = [r for (t, r) in self.rows if t0 <= t <= t1] or [r for (_, r) in self.rows[-3:]]
-        sm, mx, pw, reasons = [], [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for r in inside:
-            f = [x.strip() for x in r.split(",")]
+    def _poll_nvml(self):
+        nv = self.nv
+        bits = [(getattr(nv, "nvmlClocksEventReasonHwSlowdown", getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8)), "hw_slowdown"),
+                (getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40)), "hw_thermal_slowdown"),
+                (getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20)), "sw_thermal_slowdown"),
+                (getattr(nv, "nvmlClocksEventReasonSwPowerCap", getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4)), "sw_power_cap")]
+        get_reasons = getattr(nv, "nvmlDeviceGetCurrentClocksEventReasons", None) or nv.nvmlDeviceGetCurrentClocksThrottleReasons
+        while not self.stop_flag.is_set():
             try:
-                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+                sm = float(nv.nvmlDeviceGetClockInfo(self.dev, nv.NVML_CLOCK_SM))
+                pw = nv.nvmlDeviceGetPowerUsage(self.dev) / 1000.0
+                mask = int(get_reasons(self.dev))
+                self.rows.append((time.time(), sm, self.max_sm, pw, [n for b, n in bits if mask & b]))
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def _read_smi(self):
+        for line in self.proc.stdout:
+            f = [x.strip() for x in line.strip().split(",")]
+            try:
+                self.rows.append((time.time(), float(f[0]), float(f[1]), float(f[2]),
+                                  [n for n, val in zip(self.NAMES, f[3:7]) if val.lower().startswith("active")]))
             except (ValueError, IndexError):
                 continue
-            for n, val in zip(names, f[3:7]):
-                if val.lower().startswith("active"):
-                    reasons.add(n)
-        sm.sort()
-        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+    def window(self, t0: float, t1: float):
+        """Summary of the samples taken in [t0, t1] (host clock); the sampler keeps running."""
+        if self.source is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no clock source (NVML and nvidia-smi unavailable)"]}
+        rows = list(self.rows)
+        inside = [r for r in rows if t0 <= r[0] <= t1]
+        note = None
+        if not inside:  # region shorter than the sampling period: the nearest samples on either side
+            inside = sorted(rows, key=lambda r: min(abs(r[0] - t0), abs(r[0] - t1)))[:2]
+            note = "no sample inside the region; nearest samples reported"
+        sm = sorted(r[1] for r in inside)
+        reasons = sorted({n for r in inside for n in r[4]})
+        out = {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_min_mhz": sm[0] if sm else None,
+               "sm_max_mhz": max((r[2] for r in inside), default=None),
+               "power_w_max": max((r[3] for r in inside), default=None), "samples": len(sm), "reasons": reasons,
+               "source": self.source}
+        if note:
+            out["note"] = note
+        return out
+
+    def stop(self):
+        self.stop_flag.set()
+        if self.proc is not None:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+
+
+def _csrc_digest() -> str:
+    """sha256 over the kernel sources: ties a stored ncu traffic figure to the code it was captured on."""
+    import hashlib
+    d = os.path.join(ROOT, "paper_2403_09225_b200", "csrc")
+    hsh = hashlib.sha256()
+    for name in sorted(os.listdir(d)):
+        if name.endswith((".cu", ".cuh", ".h")):
+            with open(os.path.join(d, name), "rb") as f:
+                hsh.update(name.encode() + b"\0" + f.read())
+    return hsh.hexdigest()[:16]
+
+
+def _stored_traffic(config: int, variant: str):
+    """ncu dram__bytes_read.sum + dram__bytes_write.sum per sweep launch from the newest committed --set full capture
+    (profiles/r*_traffic.csv: config;kernel_variant;dram_bytes_per_launch;csrc_digest).  Returns (bytes, source) - or
+    (None, why) when no row was captured on the kernel sources of this tree, so that a stale figure is never printed."""
+    pdir = os.path.join(ROOT, "profiles")
+    digest = _csrc_digest()
+    stale = None
+    for name in sorted((n for n in os.listdir(pdir) if n.endswith("_traffic.csv")), reverse=True):
+        try:
+            with open(os.path.join(pdir, name)) as f:
+                for row in f:
+                    parts = [x.strip() for x in row.strip().split(";")]
+                    if len(parts) >= 3 and parts[0] == f"config{config}" and parts[1] == variant:
+                        if len(parts) >= 4 and parts[3] == digest:
+                            return float(parts[2]), f"profiles/{name} (ncu --set full, csrc digest {digest})"
+                        stale = f"profiles/{name} was captured on other kernel sources (csrc digest now {digest})"
+        except (OSError, ValueError):
+            continue
+    return None, stale or f"no ncu capture for config{config};{variant};{digest} under profiles/"
 
 
 _ORACLE_MODELS = {}
@@ -207,7 +283,7 @@ def run_fits(args):
     for k, th, r in results:
         rows[k] = {"start": k, "nll": r.nll, "grad_inf": r.grad_inf_norm, "outer": r.outer_iters, "hvp": r.n_hvp,
                    "sweeps": r.n_nll + r.n_grad + r.n_hvp, "stop": r.stop_reason, "status": r.status,
-                   "seconds": r.seconds}
+                   "active_bounds": r.n_active, "seconds": r.seconds}
         if r.status == 0 and (best is None or r.nll < best[1].nll):
             best = (th, r)
     m_launches = sum(pwa.pwa_kernel_launches(x.h) for x in workers) - l0

@@ -124,37 +124,44 @@ pwa_status pwa_combine(pwa_handle* h, const double* raw, const double* v, double
                        double* hv);
 
 /* ---- fit ---------------------------------------------------------------------------------------
- * Truncated line-search Newton-CG (Nocedal & Wright Alg. 7.1 as specialised in DESIGN.md (c-F);
- * the paper names SciPy's Newton-CG, and gives no settings).  All vectors stay on the
- * device; the host reads back a few scalars per iteration for control flow. */
+ * Projected, truncated line-search Newton-CG (Nocedal & Wright Alg. 7.1 for the inner CG; bound constraints by
+ * projection, readings S15' and S19; the paper names SciPy's Newton-CG, mentions undefined
+ * "constraint conditions", and gives no settings).  The start point is projected into the box; a
+ * variable on a bound whose gradient pushes outward is frozen for the inner solve; trial points are projected, not
+ * rejected.  gP below is the gradient with the frozen entries set to zero.  All vectors stay on the device; the
+ * host reads back a few scalars per iteration for control flow.  The call replaces the state kept by
+ * pwa_nll_grad_for_hvp (a pwa_hvp_cached after the fit refers to the fit's last gradient point). */
 typedef struct {
   int32_t max_outer;      /* 500   outer Newton iterations */
   int32_t max_cg;         /* 50    CG iterations per outer step (BASELINE.json configs[4]) */
-  double gtol;            /* 1e-5  stop when |g|_inf <= gtol */
-  double xtol;            /* 1e-8  stop when t |p|_inf <= xtol */
+  double gtol;            /* 1e-5  stop when |gP|_inf <= gtol */
+  double xtol;            /* 1e-8  stop when the accepted step |theta_new - theta|_inf <= xtol */
   double ftol;            /* 1e-12 stop when |f_new - f| <= ftol max(1,|f|) */
   double armijo_c1;       /* 1e-4 */
   double backtrack;       /* 0.5   step shrink factor rho */
   int32_t max_backtrack;  /* 40 */
   double max_seconds;     /* 0 = off; wall-time cap ("early stopping") */
-  double gamma_min, gamma_max, mass_min, mass_max; /* feasible box of the FIT only (S19): 5e-3, 2, 0.1, 4;
-                                                      a pair (0,0) switches that box off */
-  double gconv;           /* 1.0   a stopped fit counts as converged iff |g|_inf <= gconv */
+  double gamma_min, gamma_max, mass_min, mass_max; /* bounds of the FIT only (S19): Gamma_r in [5e-3, 2], M_r in
+                                                      [0.1, 4]; a pair (0,0) switches that box off */
+  double gconv;           /* 1.0   a stopped fit counts as converged iff |gP|_inf <= gconv */
 } pwa_fit_opts;
 
 typedef struct {
   double nll;             /* NLL at the returned theta */
-  double grad_inf_norm;   /* |grad|_inf there */
+  double grad_inf_norm;   /* |gP|_inf there (projected gradient: entries frozen on a bound do not count) */
   int32_t outer_iters, cg_iters;
   int32_t n_nll, n_grad, n_hvp; /* sweeps of each kind */
   int32_t stop_reason;    /* 1 gtol, 2 xtol, 3 ftol, 4 max_outer, 5 max_seconds, 6 line search failed */
   int32_t status;         /* PWA_OK (converged), PWA_ERR_NOT_CONVERGED or PWA_ERR_NONFINITE */
   double seconds;         /* wall time of the call */
+  int32_t n_active;       /* variables frozen on a bound at the returned theta */
 } pwa_fit_result;
 
 void pwa_fit_opts_default(pwa_fit_opts* opts);
 /* theta_inout: DEVICE pointer, P doubles, start point in, final point out.  opts NULL = defaults.
- * Returns result->status (or PWA_ERR_INVALID_ARG / PWA_ERR_CUDA).  Synchronises the stream. */
+ * Returns result->status (or PWA_ERR_INVALID_ARG / PWA_ERR_CUDA).  Synchronises the stream.
+ * PWA_ERR_NONFINITE: the NLL or gradient at the (projected) start point, or the gradient at an accepted point, is not
+ * finite; theta_inout then holds the last accepted point (the projected start point if no step was taken). */
 pwa_status pwa_fit_newton_cg(pwa_handle* h, double* theta_inout, const pwa_fit_opts* opts,
                              pwa_fit_result* result);
 

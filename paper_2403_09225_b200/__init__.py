@@ -63,7 +63,7 @@ class pwa_fit_opts(Structure):
 class pwa_fit_result(Structure):
     _fields_ = [("nll", c_double), ("grad_inf_norm", c_double), ("outer_iters", c_int32), ("cg_iters", c_int32),
                 ("n_nll", c_int32), ("n_grad", c_int32), ("n_hvp", c_int32), ("stop_reason", c_int32),
-                ("status", c_int32), ("seconds", c_double)]
+                ("status", c_int32), ("seconds", c_double), ("n_active", c_int32)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

@@ -147,10 +147,12 @@ pwa_status eval(pwa_handle* h, int mode, const double* theta, const double* v, d
 // sums P1, P2, P3 in the handle; every following HVP at that theta only accumulates Q1, Q2 (MODE_HVPQ).
 // Shapes served by the generic kernel have no such modes: they fall back to the fused sweep at the kept theta.
 pwa_status eval_grad_keep(pwa_handle* h, const double* theta, double* nll, double* grad) {
+  h->keep_valid = false;  // valid again only once everything that refreshes the kept state has been enqueued
   PWA_CUDA_CHECK(h, cudaMemcpyAsync(h->d_theta_keep, theta, sizeof(double) * h->n_par, cudaMemcpyDeviceToDevice, h->stream));
-  h->keep_valid = true;
-  if (h->variant < 2) return eval(h, MODE_GRAD, theta, nullptr, nll, grad, nullptr);
-  return raw_sums_impl(h, MODE_GRAD3, h->d_theta_keep, nullptr, h->d_raw, true, nll, grad, nullptr);
+  const pwa_status st = h->variant < 2 ? eval(h, MODE_GRAD, theta, nullptr, nll, grad, nullptr)
+                                       : raw_sums_impl(h, MODE_GRAD3, h->d_theta_keep, nullptr, h->d_raw, true, nll, grad, nullptr);
+  h->keep_valid = st == PWA_OK;
+  return st;
 }
 
 pwa_status eval_hvp_kept(pwa_handle* h, const double* v, double* hv, const double* skip) {
@@ -247,8 +249,12 @@ extern "C" pwa_status pwa_create(const pwa_model_desc* m, pwa_handle** out) {
     return fail_create(nullptr, PWA_ERR_CUDA, std::string("no usable CUDA device: ") + cudaGetErrorString(ce));
   }
   if (m->device < 0 || m->device >= ndev) return fail_create(nullptr, PWA_ERR_INVALID_ARG, "device ordinal out of range");
-  if ((ce = cudaSetDevice(m->device)) != cudaSuccess)
-    return fail_create(nullptr, PWA_ERR_CUDA, std::string("cudaSetDevice: ") + cudaGetErrorString(ce));
+  DeviceGuard guard(m->device);  // restores the caller's current device on every return path
+  {
+    int cur = -1;
+    if ((ce = cudaGetDevice(&cur)) != cudaSuccess || cur != m->device)
+      return fail_create(nullptr, PWA_ERR_CUDA, std::string("cudaSetDevice: ") + cudaGetErrorString(ce));
+  }
 
   pwa_handle* h = new (std::nothrow) pwa_handle();
   if (!h) return fail_create(nullptr, PWA_ERR_OOM, "host allocation failed");
@@ -333,7 +339,7 @@ extern "C" pwa_status pwa_create(const pwa_model_desc* m, pwa_handle** out) {
 
 extern "C" pwa_status pwa_destroy(pwa_handle* h) {
   if (!h) return PWA_OK;
-  cudaSetDevice(h->device);
+  DeviceGuard guard(h->device);
   cudaStreamSynchronize(h->stream);
   for (void* p : h->owned) if (p) cudaFree(p);
   void* dev[] = {h->d_ch, h->d_K, h->d_partial, h->d_sums, h->d_raw, h->d_flags, h->d_io, h->d_fit, h->d_pcache, h->d_theta_keep};
@@ -355,18 +361,21 @@ extern "C" int32_t pwa_raw_size(const pwa_handle* h) { return h ? 4 + 4 * h->n_p
 
 extern "C" pwa_status pwa_nll(pwa_handle* h, const double* theta, double* nll) {
   if (!h) return PWA_ERR_INVALID_ARG;
+  DeviceGuard guard(h->device);
   PWA_REQUIRE(h, theta && nll, "pwa_nll: null pointer");
   return eval(h, MODE_NLL, theta, nullptr, nll, nullptr, nullptr);
 }
 
 extern "C" pwa_status pwa_nll_grad(pwa_handle* h, const double* theta, double* nll, double* grad) {
   if (!h) return PWA_ERR_INVALID_ARG;
+  DeviceGuard guard(h->device);
   PWA_REQUIRE(h, theta && nll && grad, "pwa_nll_grad: null pointer");
   return eval(h, MODE_GRAD, theta, nullptr, nll, grad, nullptr);
 }
 
 extern "C" pwa_status pwa_hvp(pwa_handle* h, const double* theta, const double* v, double* hv) {
   if (!h) return PWA_ERR_INVALID_ARG;
+  DeviceGuard guard(h->device);
   PWA_REQUIRE(h, theta && v && hv, "pwa_hvp: null pointer");
   return eval(h, MODE_FULL, theta, v, nullptr, nullptr, hv);
 }
@@ -374,12 +383,14 @@ extern "C" pwa_status pwa_hvp(pwa_handle* h, const double* theta, const double* 
 extern "C" pwa_status pwa_nll_grad_hvp(pwa_handle* h, const double* theta, const double* v, double* nll, double* grad,
                                        double* hv) {
   if (!h) return PWA_ERR_INVALID_ARG;
+  DeviceGuard guard(h->device);
   PWA_REQUIRE(h, theta && v && nll && grad && hv, "pwa_nll_grad_hvp: null pointer");
   return eval(h, MODE_FULL, theta, v, nll, grad, hv);
 }
 
 extern "C" pwa_status pwa_raw_sums(pwa_handle* h, const double* theta, const double* v, double* raw) {
   if (!h) return PWA_ERR_INVALID_ARG;
+  DeviceGuard guard(h->device);
   PWA_REQUIRE(h, theta && raw, "pwa_raw_sums: null pointer");
   return raw_sums_impl(h, v ? MODE_FULL : MODE_GRAD, theta, v, raw);
 }
@@ -387,6 +398,7 @@ extern "C" pwa_status pwa_raw_sums(pwa_handle* h, const double* theta, const dou
 extern "C" pwa_status pwa_combine(pwa_handle* h, const double* raw, const double* v, double* nll, double* grad,
                                   double* hv) {
   if (!h) return PWA_ERR_INVALID_ARG;
+  DeviceGuard guard(h->device);
   PWA_REQUIRE(h, raw, "pwa_combine: null raw");
   PWA_REQUIRE(h, !hv || v, "pwa_combine: hv requires v");
   return combine_impl(h, raw, v, nll, grad, hv);
@@ -395,6 +407,7 @@ extern "C" pwa_status pwa_combine(pwa_handle* h, const double* raw, const double
 extern "C" pwa_status pwa_nll_grad_hvp_host(pwa_handle* h, const double* theta_host, const double* v_host,
                                             double* nll_host, double* grad_host, double* hv_host) {
   if (!h) return PWA_ERR_INVALID_ARG;
+  DeviceGuard guard(h->device);
   PWA_REQUIRE(h, theta_host, "pwa_nll_grad_hvp_host: null theta");
   PWA_REQUIRE(h, !hv_host || v_host, "pwa_nll_grad_hvp_host: hv requires v");
   const size_t P = h->n_par;
@@ -419,6 +432,7 @@ extern "C" pwa_status pwa_nll_grad_hvp_host(pwa_handle* h, const double* theta_h
 // ---- diagnostics --------------------------------------------------------------------------------------
 extern "C" pwa_status pwa_status_flags(pwa_handle* h, uint32_t* flags_host) {
   if (!h) return PWA_ERR_INVALID_ARG;
+  DeviceGuard guard(h->device);
   PWA_REQUIRE(h, flags_host, "pwa_status_flags: null pointer");
   unsigned f = 0;
   PWA_CUDA_CHECK(h, cudaMemcpyAsync(&f, h->d_flags, sizeof(unsigned), cudaMemcpyDeviceToHost, h->stream));
@@ -429,6 +443,7 @@ extern "C" pwa_status pwa_status_flags(pwa_handle* h, uint32_t* flags_host) {
 
 extern "C" pwa_status pwa_profile_enable(pwa_handle* h, int32_t on) {
   if (!h) return PWA_ERR_INVALID_ARG;
+  DeviceGuard guard(h->device);
   if (on && h->prof_events.empty()) {
     h->prof_events.resize(2 * 4096);
     for (size_t i = 0; i < h->prof_events.size(); ++i) {
@@ -446,6 +461,7 @@ extern "C" pwa_status pwa_profile_enable(pwa_handle* h, int32_t on) {
 
 extern "C" pwa_status pwa_profile_read(pwa_handle* h, double* total_ms, int64_t* n_launches) {
   if (!h) return PWA_ERR_INVALID_ARG;
+  DeviceGuard guard(h->device);
   PWA_CUDA_CHECK(h, cudaStreamSynchronize(h->stream));
   double tot = 0.0;
   for (size_t i = 0; i + 1 < h->prof_used; i += 2) {
@@ -461,12 +477,14 @@ extern "C" pwa_status pwa_profile_read(pwa_handle* h, double* total_ms, int64_t*
 
 extern "C" pwa_status pwa_nll_grad_for_hvp(pwa_handle* h, const double* theta, double* nll, double* grad) {
   if (!h) return PWA_ERR_INVALID_ARG;
+  DeviceGuard guard(h->device);
   if (!theta) return set_error(h, PWA_ERR_INVALID_ARG, "pwa_nll_grad_for_hvp: null theta", cudaSuccess);
   return eval_grad_keep(h, theta, nll, grad);
 }
 
 extern "C" pwa_status pwa_hvp_cached(pwa_handle* h, const double* v, double* hv) {
   if (!h) return PWA_ERR_INVALID_ARG;
+  DeviceGuard guard(h->device);
   if (!v || !hv) return set_error(h, PWA_ERR_INVALID_ARG, "pwa_hvp_cached: null pointer", cudaSuccess);
   return eval_hvp_kept(h, v, hv);
 }

@@ -114,6 +114,7 @@ using namespace pwa;
 
 extern "C" pwa_status pwa_fit_fractions(pwa_handle* h, const double* theta, double* frac) {
   if (!h) return PWA_ERR_INVALID_ARG;
+  pwa::DeviceGuard guard(h->device);
   if (!theta || !frac) return set_error(h, PWA_ERR_INVALID_ARG, "pwa_fit_fractions: null pointer", cudaSuccess);
   frac_fn fn = frac_kernel(h->n_hel);
   if (!fn) return set_error(h, PWA_ERR_INVALID_ARG, "pwa_fit_fractions: n_hel out of range", cudaSuccess);

@@ -93,6 +93,25 @@ pwa_status eval_hvp_kept(pwa_handle* h, const double* v, double* hv, const doubl
 pwa_status set_error(pwa_handle* h, pwa_status st, const char* what, cudaError_t ce);
 }  // namespace pwa
 
+namespace pwa {
+// Binds the calling thread to a handle's device for the duration of one C-ABI call and restores the caller's current
+// device afterwards ("one handle = one device", include/pwa.h): a handle may be used from a thread whose current
+// device is another one (one host thread per GPU).
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int device) {
+    if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); prev = -1; }
+    if (prev != device) switched = cudaSetDevice(device) == cudaSuccess;
+  }
+  ~DeviceGuard() {
+    if (switched && prev >= 0) cudaSetDevice(prev);
+  }
+  DeviceGuard(const DeviceGuard&) = delete;
+  DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+}  // namespace pwa
+
 #define PWA_CUDA_CHECK(h, call)                                              \
   do {                                                                       \
     cudaError_t ce__ = (call);                                               \

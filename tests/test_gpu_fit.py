@@ -7,7 +7,10 @@ raw theta is never compared.  What is unique and compared:
     shift a CG exit by an iteration);
   * at the point the CUDA fit returns, the ORACLE's gradient is small and its NLL equals the reported one
     (north_star tolerances): the result is checked by the oracle, not by the kernel that produced it;
-  * the NLL never increased (Armijo) and the S19 box holds at the returned point;
+  * the NLL never increased (Armijo) and the S19 box holds at the returned point; with a box that cuts the free
+    minimum off both sides end on the same bounds with the same NLL (projected Newton-CG, DESIGN.md S15');
+  * fits run to their own stop from 12 random starts on both sides: same convergence class, same NLL where the
+    trajectories stay together; starts that rounding sends to different basins (PAPER.md:133) are counted and bounded;
   * a start with a non-finite NLL (all couplings zero: ln 0) is reported as PWA_ERR_NONFINITE.
 """
 import numpy as np
@@ -80,6 +83,88 @@ def test_fit_from_random_starts_follows_the_reference(oracle_mod, setup):
         assert res.outer_iters == ref.outer_iters and res.stop_reason == ref.stop_reason
         f0 = float(oracle_mod.nll(om, th, "ld"))
         assert abs(f0 - res.nll) <= 1e-10 * max(1.0, abs(f0))
+
+
+def test_active_bounds_match_the_reference_fit(oracle_mod, setup):
+    """A box that cuts the unconstrained minimum off (widths capped below the fitted ones, a mass floor above a fitted
+    mass): both sides must end on the same bounds, with the same NLL, and the oracle's projected gradient at the CUDA
+    point must vanish while the frozen entries push outward (KKT)."""
+    from oracle.fit import FitOpts, bounds, fit_newton_cg, projected_gradient
+    pwa, workloads, models = setup
+    cfg, w, om, gm = models[1]
+    th0 = workloads.theta_true(cfg).numpy()
+    th_free, r_free = gm.fit(th0)
+    assert r_free.status == 0 and r_free.n_active == 0
+    gmax, mmin = 0.8 * float(th_free[3::4].min()), float(th_free[2::4].min()) + 0.02
+    ref = fit_newton_cg(om, th0, FitOpts(gamma_max=gmax, mass_min=mmin), prec="d", threads=oracle_mod.max_threads())
+    th, res = gm.fit(th0, _opts(pwa, gamma_max=gmax, mass_min=mmin))
+    assert ref.converged and res.status == 0 and res.n_active == ref.n_active >= 2
+    assert abs(res.nll - ref.nll) <= 1e-7 * max(1.0, abs(ref.nll)) and res.nll > r_free.nll
+    lo, hi = bounds(len(th), FitOpts(gamma_max=gmax, mass_min=mmin))
+    assert np.all(th >= lo) and np.all(th <= hi)
+    assert np.array_equal(th <= lo, np.asarray(ref.theta, dtype=np.float64) <= lo)
+    assert np.array_equal(th >= hi, np.asarray(ref.theta, dtype=np.float64) >= hi)
+    _, g0, _ = oracle_mod.nll_grad_hvp(om, th, None, "ld")
+    g0 = np.asarray(g0, dtype=np.float64)
+    gP, free = projected_gradient(th, g0, lo, hi)
+    assert float(np.max(np.abs(gP))) <= max(10 * res.grad_inf_norm, 1e-3)
+    assert np.all(g0[~free & (th <= lo)] > 0) and np.all(g0[~free & (th >= hi)] < 0)
+
+
+def test_start_outside_the_box_is_projected(setup):
+    pwa, workloads, models = setup
+    cfg, w, om, gm = models[1]
+    th0 = workloads.theta_true(cfg).numpy().copy()
+    th0[3] = 5.0
+    th0[6] = 0.01
+    o = _opts(pwa, max_outer=0)
+    th, res = gm.fit(th0, o)
+    assert th[3] == o.gamma_max and th[6] == o.mass_min and res.stop_reason == 4
+    want = th0.copy(); want[3] = o.gamma_max; want[6] = o.mass_min
+    assert np.array_equal(th, want) and abs(res.nll - gm.nll(th)) <= 1e-13 * abs(res.nll)  # different kernel modes
+
+
+@pytest.mark.parametrize("idx,n_starts", [(1, 8), (2, 4)])
+def test_fits_to_completion_on_both_sides(oracle_mod, setup, idx, n_starts, capsys):
+    """north_star: "Newton-CG fits reach the oracle's minimum".  Both sides run the SAME algorithm (S15') from the same
+    random starts (S16) to their own stop.  Required of every start: the same convergence class, the CUDA value equal to
+    the oracle's NLL at the CUDA point, and - where the CUDA fit converged - a vanishing oracle projected gradient
+    there.  Where both converge the final NLLs agree to 1e-6 relative unless rounding has sent the two trajectories
+    (100+ iterations through saddle regions) into different local minima, which PAPER.md:133 describes; those starts
+    are printed.  On the config-1 shape (P = 8) they must stay a minority (measured: 0 of 8).  On the config-2 shape
+    (P = 40 on 3 000 data events: dozens of local minima) the oracle's own end point changes with its OpenMP thread
+    count (start 1: -1688.68 on 8 threads, -1692.18 on 16), so per-start agreement is not a property of either
+    side there (measured: 1 of 4 agree); what is required is that every CUDA end point is a KKT point by the oracle."""
+    from oracle.fit import FitOpts, bounds, fit_newton_cg, projected_gradient
+    pwa, workloads, models = setup
+    cfg, w, om, gm = models[idx]
+    nt = oracle_mod.max_threads()
+    lo, hi = bounds(cfg.n_par, FitOpts())
+    same, different, rows = 0, [], []
+    for k in range(n_starts):
+        th0 = workloads.random_start(cfg, k).numpy()
+        ref = fit_newton_cg(om, th0, FitOpts(), prec="d", threads=nt)
+        th, res = gm.fit(th0)
+        rows.append((k, ref.nll, ref.stop_reason, ref.converged, res.nll, res.stop_reason, res.status))
+        assert (res.status == 0) == ref.converged, rows[-1]
+        f0, g0, _ = oracle_mod.nll_grad_hvp(om, th, None, "d", threads=nt)
+        assert abs(float(f0) - res.nll) <= 1e-10 * max(1.0, abs(float(f0)))
+        assert np.all(th >= lo) and np.all(th <= hi)
+        if res.status == 0:
+            gP, _ = projected_gradient(th, np.asarray(g0, dtype=np.float64), lo, hi)
+            assert float(np.max(np.abs(gP))) <= FitOpts().gconv
+            if abs(res.nll - ref.nll) <= 1e-6 * max(1.0, abs(ref.nll)):
+                same += 1
+                assert res.stop_reason in (1, 2, 3) and ref.stop_reason in (1, 2, 3)
+            else:
+                different.append(k)
+    with capsys.disabled():
+        print(f"\nconfig-{idx} shape, {n_starts} random starts: {same} end at the reference fit's NLL, "
+              f"different basins: {different}")
+        for r in rows:
+            print("  start %d: oracle nll %.6f stop %d conv %s | cuda nll %.6f stop %d status %d" % r)
+    if idx == 1:
+        assert len(different) <= n_starts // 2
 
 
 def test_nonfinite_start_is_reported(setup):
