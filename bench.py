@@ -30,6 +30,9 @@ if ROOT not in sys.path:
 
 METRIC = "nll_grad_hvp_events_per_s"
 UNIT = "events/s"
+# entry points a step can call (--mode); the metric's step is the fused sweep
+MODES = {"nll_grad_hvp": "pwa_nll_grad_hvp", "nll": "pwa_nll", "nll_grad": "pwa_nll_grad",
+         "nll_grad_for_hvp": "pwa_nll_grad_for_hvp", "hvp_cached": "pwa_hvp_cached", "hvp": "pwa_hvp"}
 
 
 def _peaks():
@@ -329,7 +332,15 @@ def main():
     ap.add_argument("--fits", type=int, default=20, help="--config 5: number of seeded random starts")
     ap.add_argument("--max-seconds", type=float, default=0.0, help="--config 5: wall-time cap per fit (0 = off)")
     ap.add_argument("--concurrent", type=int, default=1, help="--config 5: independent fits in flight (handles + streams)")
+    ap.add_argument("--mode", default="nll_grad_hvp", choices=list(MODES),
+                    help="entry point one step calls (default: the fused sweep, the metric's step)")
+    ap.add_argument("--sustained-seconds", type=float, default=1.2,
+                    help="length of the back-to-back run behind roofline_sustained (0 = skip)")
+    ap.add_argument("--csrc-digest", action="store_true", help="print the digest a profiles/*_traffic.csv row must carry, and exit")
     args = ap.parse_args()
+    if args.csrc_digest:
+        print(_csrc_digest())
+        return 0
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else max(args.warmup, 1)
     if args.impl == "reference":
         if args.config == 5:
@@ -375,9 +386,20 @@ def main():
     events_per_step = cfg.n_mc + cfg.n_data
     bytes_per_step = pwa.pwa_bytes_per_eval(m.h)
 
+    single = {"nll_grad_hvp": lambda: pwa.pwa_nll_grad_hvp(m.h, theta, v, m.nll_t, m.grad_t, m.hv_t),
+              "nll": lambda: pwa.pwa_nll(m.h, theta, m.nll_t),
+              "nll_grad": lambda: pwa.pwa_nll_grad(m.h, theta, m.nll_t, m.grad_t),
+              "nll_grad_for_hvp": lambda: pwa.pwa_nll_grad_for_hvp(m.h, theta, m.nll_t, m.grad_t),
+              "hvp_cached": lambda: pwa.pwa_hvp_cached(m.h, v, m.hv_t),
+              "hvp": lambda: pwa.pwa_hvp(m.h, theta, v, m.hv_t)}[args.mode]
+    if args.mode == "hvp_cached":
+        pwa.pwa_nll_grad_for_hvp(m.h, theta, m.nll_t, m.grad_t)
+    if world > 1 and args.mode != "nll_grad_hvp":
+        raise SystemExit("--mode is a one-GPU measurement")
+
     def step():
         if world == 1:
-            pwa.pwa_nll_grad_hvp(m.h, theta, v, m.nll_t, m.grad_t, m.hv_t)
+            single()
         else:
             pwa.pwa_raw_sums(m.h, theta, v, raw)
             dist.all_reduce(raw)
@@ -394,7 +416,7 @@ def main():
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-        time.sleep(0.3)
+        time.sleep(0.05)
     pwa.pwa_profile_enable(m.h, True)
     pwa.pwa_profile_read(m.h)
     l0 = pwa.pwa_kernel_launches(m.h)
@@ -411,7 +433,7 @@ def main():
     sweep_ms, sweep_n = pwa.pwa_profile_read(m.h)
     pwa.pwa_profile_enable(m.h, False)
     launches = pwa.pwa_kernel_launches(m.h) - l0
-    clocks = sampler.stop(tw0, tw1) if rank == 0 else None
+    clocks = sampler.window(tw0, tw1) if rank == 0 else None
     if world > 1:
         t = torch.tensor([ms], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -458,6 +480,38 @@ def main():
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         e2e_s = float(t.item())
 
+    # ---- sustained: >= --sustained-seconds of back-to-back steps AFTER the timed region (fits are seconds of
+    # back-to-back sweeps; the SM clock sags under the FP64 load after some tens of milliseconds).
+    # Per-launch sweep times from the library's CUDA events on the launching stream; the mean of the last half counts.
+    sustained = None
+    if args.sustained_seconds > 0 and world == 1:
+        n_long = int(min(4000, max(50, args.sustained_seconds / (ms / args.steps * 1e-3))))
+        pwa.pwa_profile_enable(m.h, True)
+        pwa.pwa_profile_read(m.h)
+        torch.cuda.synchronize()
+        half = n_long // 2
+        ts0 = time.time()
+        e_a, e_b, e_c = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        e_a.record()
+        for _ in range(half):
+            step()
+        e_b.record()
+        torch.cuda.synchronize()
+        first_ms, first_n = pwa.pwa_profile_read(m.h)
+        ts1 = time.time()
+        for _ in range(n_long - half):
+            step()
+        e_c.record()
+        torch.cuda.synchronize()
+        ts2 = time.time()
+        last_ms, last_n = pwa.pwa_profile_read(m.h)
+        pwa.pwa_profile_enable(m.h, False)
+        sustained = {"first": (first_ms / max(first_n, 1), e_a.elapsed_time(e_b) / half),
+                     "last": (last_ms / max(last_n, 1), e_b.elapsed_time(e_c) / (n_long - half)),
+                     "n": n_long, "seconds": ts2 - ts0, "clocks": sampler.window(ts1, ts2)}
+    if rank == 0:
+        sampler.stop()
+
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -466,18 +520,8 @@ def main():
     peak, peak_src = _peaks()
     sweep_avg_s = (sweep_ms / max(sweep_n, 1)) * 1e-3
     achieved = bytes_per_step / sweep_avg_s / 1e9 if sweep_n else None
-    traffic = None
-    # ncu dram__bytes_read.sum + dram__bytes_write.sum per sweep launch, copied from the committed --set full capture
-    tpath = os.path.join(ROOT, "profiles", "r01_traffic.csv")  # columns: config,kernel_variant,dram_bytes_per_launch
-    if os.path.exists(tpath):
-        try:
-            with open(tpath) as f:
-                for row in f:
-                    parts = [x.strip() for x in row.strip().split(";")]
-                    if len(parts) == 3 and parts[0] == f"config{args.config}" and parts[1] == pwa.pwa_kernel_variant(m.h):
-                        traffic = float(parts[2])
-        except Exception:
-            traffic = None
+    traffic, traffic_src = (None, "stored figures are for the fused sweep") if args.mode != "nll_grad_hvp" else \
+        _stored_traffic(args.config, pwa.pwa_kernel_variant(m.h))
     line = {
         "metric": METRIC, "value": world * events_per_step * args.steps / (ms * 1e-3), "unit": UNIT,
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
@@ -488,12 +532,13 @@ def main():
                    "l2": f"inputs ({bytes_per_step / 1e6:.0f} MB per step) exceed the 126 MB L2; no flush needed"
                          if bytes_per_step > 2 * 126e6 else "inputs fit in L2 (cache-resident case)",
                    "kernel_variant": pwa.pwa_kernel_variant(m.h), "parallelism": f"event shards x{world}",
+                   "entry_point": MODES[args.mode],
                    "workload_gen_s": round(t_gen, 1)},
         "evals_per_s": args.steps / (ms * 1e-3),
         "nll": nll_dev,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": (achieved / peak) if achieved else None, "traffic": traffic,
-                     "peak_source": peak_src, "kernel": "sweep", "bytes_per_launch": bytes_per_step,
+                     "traffic_source": traffic_src, "peak_source": peak_src, "kernel": "sweep", "bytes_per_launch": bytes_per_step,
                      "avg_launch_ms": sweep_avg_s * 1e3, "launches_timed": sweep_n},
         "e2e": {"value": world * events_per_step * args.steps / e2e_s, "unit": UNIT,
                 "h2d_bytes_per_step": 2 * P * 8, "d2h_bytes_per_step": (1 + 2 * P) * 8,
@@ -501,14 +546,27 @@ def main():
         "gpu_launches": int(launches),
         "clocks": clocks,
     }
+    if sustained is not None:
+        k_ms, step_ms = sustained["last"]
+        ach = bytes_per_step / (k_ms * 1e-3) / 1e9
+        line["roofline_sustained"] = {
+            "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+            "avg_launch_ms": k_ms, "ms_per_step": step_ms, "launches": sustained["n"],
+            "seconds": round(sustained["seconds"], 3),
+            "first_half": {"avg_launch_ms": sustained["first"][0], "frac": bytes_per_step / (sustained["first"][0] * 1e-3) / 1e9 / peak},
+            "what": f"{sustained['n']} back-to-back steps right after the timed region; per-launch CUDA events of the sweep "
+                    "kernel; achieved = algorithmic bytes / mean launch time of the LAST half",
+            "peak_source": peak_src, "clocks": sustained["clocks"]}
     # the ALU co-limit beside the HBM roofline: FP64 instructions the method needs per event
     # (16 R H + 52 R + 80 DFMA-class) against the FP64 pipe rate measured on this pool
     # (profiles/r01_microbench.md: 17.05 T DFMA/s sustained)
     fp64_per_event = 16 * cfg.n_res * cfg.n_hel + 52 * cfg.n_res + 80
     if sweep_n:
         rate = fp64_per_event * events_per_step / sweep_avg_s / 1e12
-        line["fp64_pipe"] = {"dfma_class_per_event": fp64_per_event, "achieved": rate, "peak": 17.05,
-                             "unit": "T instr/s", "frac": rate / 17.05,
+        line["fp64_pipe"] = {"dfma_class_per_event_estimate": fp64_per_event, "achieved_estimate": rate, "peak": 17.05,
+                             "unit": "T instr/s", "frac_estimate": rate / 17.05,
+                             "note": "instruction count is SURVEY 8(d)'s formula 16RH + 52R + 80, not an executed count; "
+                                     "the executed FP64-pipe activity is ncu's (profiles/, sweep_full)",
                              "peak_source": "measured (profiles/r01_microbench.md, fp64_peak)"}
     if not args.no_cpu_baseline:
         import oracle
