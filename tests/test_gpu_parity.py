@@ -299,3 +299,33 @@ def test_hvp_cached_needs_a_keeping_call(pwa, oracle_mod):
         assert e.value.status == 1
     finally:
         gm.close()
+
+
+@pytest.mark.parametrize("idx,n_mc,n_data", [CASES[1], CASES[2]])
+def test_unconstrained_parameter_domain(pwa, oracle_mod, idx, n_mc, n_data):
+    """Reading S7: the evaluation calls take unconstrained reals.  One coupling exactly zero among non-zero
+    ones (its d/da entry stays finite and non-zero: e^{i phi} B S), a negative modulus, a negative width (the pole moves
+    to the other half plane), phases of order 1e3 (sincos argument reduction) - every entry point against the oracle."""
+    import workloads
+    cfg, w, om, gm = _case(pwa, oracle_mod, idx, n_mc, n_data)
+    base = workloads.random_start(cfg, 2).numpy()
+    v = workloads.direction(cfg, 6).numpy()
+    variants = {}
+    t = base.copy(); t[4 * 1] = 0.0; variants["a_1 = 0"] = t
+    t = base.copy(); t[4 * 0] = -t[4 * 0]; t[4 * 2] = -0.37; variants["a < 0"] = t
+    t = base.copy(); t[4 * 1 + 3] = -t[4 * 1 + 3]; variants["Gamma_1 < 0"] = t
+    t = base.copy(); t[1::4] += 1000.0 * np.where(np.arange(cfg.n_res) % 2 == 0, 1.0, -1.0); variants["|phi| ~ 1e3"] = t
+    t = base.copy(); t[4 * 1] = 0.0; t[4 * 0] = -1.2; t[4 * 2 + 3] = -0.11; t[1::4] -= 777.0; variants["all at once"] = t
+    for name, th in variants.items():
+        f0, g0, h0 = oracle_mod.nll_grad_hvp(om, th, v, "ld")
+        f, g, hv = gm.nll_grad_hvp(th, v)
+        assert _nll_err(f, f0) < NLL_TOL, (name, f, float(f0))
+        assert rel_l2(g, g0) < VEC_TOL and rel_l2(hv, h0) < VEC_TOL, name
+        assert pwa.pwa_status_flags(gm.h) == 0, name
+        assert _nll_err(gm.nll(th), f0) < NLL_TOL, name
+        f1, g1 = gm.nll_grad_for_hvp(th)
+        assert _nll_err(f1, f0) < NLL_TOL and rel_l2(g1, g0) < VEC_TOL, name
+        assert rel_l2(gm.hvp_cached(v), h0) < VEC_TOL, name
+        if name == "a_1 = 0":
+            assert g[4] != 0.0 and np.isfinite(g[4])
+            assert abs(g[4] - float(g0[4])) <= 1e-8 * abs(float(g0[4]))

@@ -46,8 +46,11 @@ def _worker(rank: int, world: int, port: int, out_dir: str):
         sm, gG, hG = oracle.raw_sums(om, "mc", th, v, "d", first=m0, count=m1 - m0)
         raw = torch.from_numpy(_pack(sd, sm, gd, gG, hd, hG))
         assert raw.numel() == sharded.RAW_HEADER + 4 * om.n_par
+        det = raw.clone()
         sharded.allreduce_raw(raw, dist)
-        r = raw.numpy()
+        sharded.allreduce_raw(det, dist, deterministic=True)   # all-gather + rank-order sum
+        assert np.allclose(det.numpy(), raw.numpy(), rtol=1e-15, atol=0.0)
+        r = det.numpy()
         P = om.n_par
         blk = lambda k: r[4 + k * P: 4 + (k + 1) * P]
         nll, grad, hv = oracle.combine(r[0:2], r[2:4], blk(0), blk(1), blk(2), blk(3), v, "d")
@@ -65,7 +68,10 @@ def test_shard_range_partitions_every_event():
             assert cuts[0][0] == 0 and cuts[-1][1] == n
             assert all(a[1] == b[0] for a, b in zip(cuts, cuts[1:]))
             sizes = [hi - lo for lo, hi in cuts]
-            assert max(sizes) - min(sizes) <= 1
+            assert max(sizes) - min(sizes) < 2 * 32
+            assert all(lo % 32 == 0 or lo == n for lo, _ in cuts)  # zero-copy windows stay 16-byte aligned per plane
+            exact = [shard_range(n, r, world, align=1) for r in range(world)]
+            assert max(hi - lo for lo, hi in exact) - min(hi - lo for lo, hi in exact) <= 1
     with pytest.raises(ValueError):
         shard_range(10, 2, 2)
 
