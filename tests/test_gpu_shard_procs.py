@@ -15,7 +15,7 @@ import torch.multiprocessing as mp
 from helpers import rel_l2
 
 pytestmark = pytest.mark.gpu
-N_MC, N_DATA = 40_013, 5_003  # ragged: the last shard ends off a tile boundary
+N_MC, N_DATA = 40_014, 5_002  # ragged (the last shard ends off a tile boundary) but even: planes of a borrowed store must be 16-byte aligned
 
 
 def _free_port() -> int:
