@@ -32,7 +32,8 @@ METRIC = "nll_grad_hvp_events_per_s"
 UNIT = "events/s"
 # entry points a step can call (--mode); the metric's step is the fused sweep
 MODES = {"nll_grad_hvp": "pwa_nll_grad_hvp", "nll": "pwa_nll", "nll_grad": "pwa_nll_grad",
-         "nll_grad_for_hvp": "pwa_nll_grad_for_hvp", "hvp_cached": "pwa_hvp_cached", "hvp": "pwa_hvp"}
+         "nll_grad_for_hvp": "pwa_nll_grad_for_hvp", "hvp_cached": "pwa_hvp_cached", "hvp": "pwa_hvp",
+         "nll_batch": "pwa_nll_batch", "hvp_cached_batch": "pwa_hvp_cached_batch"}
 
 
 def _peaks():
@@ -334,6 +335,7 @@ def main():
     ap.add_argument("--concurrent", type=int, default=1, help="--config 5: independent fits in flight (handles + streams)")
     ap.add_argument("--mode", default="nll_grad_hvp", choices=list(MODES),
                     help="entry point one step calls (default: the fused sweep, the metric's step)")
+    ap.add_argument("--batch", type=int, default=4, help="--mode nll_batch / hvp_cached_batch: evaluations per call (K)")
     ap.add_argument("--sustained-seconds", type=float, default=1.2,
                     help="length of the back-to-back run behind roofline_sustained (0 = skip)")
     ap.add_argument("--csrc-digest", action="store_true", help="print the digest a profiles/*_traffic.csv row must carry, and exit")
@@ -391,8 +393,16 @@ def main():
               "nll_grad": lambda: pwa.pwa_nll_grad(m.h, theta, m.nll_t, m.grad_t),
               "nll_grad_for_hvp": lambda: pwa.pwa_nll_grad_for_hvp(m.h, theta, m.nll_t, m.grad_t),
               "hvp_cached": lambda: pwa.pwa_hvp_cached(m.h, v, m.hv_t),
-              "hvp": lambda: pwa.pwa_hvp(m.h, theta, v, m.hv_t)}[args.mode]
-    if args.mode == "hvp_cached":
+              "hvp": lambda: pwa.pwa_hvp(m.h, theta, v, m.hv_t),
+              "nll_batch": lambda: pwa.pwa_nll_batch(m.h, args.batch, theta_k, nll_k),
+              "hvp_cached_batch": lambda: pwa.pwa_hvp_cached_batch(m.h, args.batch, v_k, hv_k)}[args.mode]
+    evals_per_step = args.batch if args.mode.endswith("_batch") else 1
+    if args.mode.endswith("_batch"):  # K parameter sets (seeded random starts) / K directions
+        theta_k = torch.tensor(np.stack([workloads.random_start(base, k).numpy() for k in range(args.batch)]), device=dev)
+        v_k = torch.tensor(np.stack([workloads.direction(base, k).numpy() for k in range(args.batch)]), device=dev)
+        nll_k = torch.zeros(args.batch, dtype=torch.float64, device=dev)
+        hv_k = torch.zeros(args.batch, P, dtype=torch.float64, device=dev)
+    if args.mode in ("hvp_cached", "hvp_cached_batch"):
         pwa.pwa_nll_grad_for_hvp(m.h, theta, m.nll_t, m.grad_t)
     if world > 1 and args.mode != "nll_grad_hvp":
         raise SystemExit("--mode is a one-GPU measurement")
@@ -534,7 +544,7 @@ def main():
                    "kernel_variant": pwa.pwa_kernel_variant(m.h), "parallelism": f"event shards x{world}",
                    "entry_point": MODES[args.mode],
                    "workload_gen_s": round(t_gen, 1)},
-        "evals_per_s": args.steps / (ms * 1e-3),
+        "evals_per_s": evals_per_step * args.steps / (ms * 1e-3), "evals_per_step": evals_per_step,
         "nll": nll_dev,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": (achieved / peak) if achieved else None, "traffic": traffic,

@@ -105,6 +105,25 @@ pwa_status pwa_nll_grad_hvp(pwa_handle* h, const double* theta, const double* v,
 pwa_status pwa_nll_grad_for_hvp(pwa_handle* h, const double* theta, double* nll, double* grad);
 pwa_status pwa_hvp_cached(pwa_handle* h, const double* v, double* hv);
 
+/* ---- K evaluations in one pass over the event store (multi-start batching; 300 fits on the same events,
+ * :133: 11+ starts per analysis; Table 1's parameter errors, :102-113, need the Hessian at the fitted point) ----------
+ * pwa_nll_batch: nll[k] = NLL(theta[k]), k < K.  theta: DEVICE pointer, K x P doubles, row k = parameter set k; nll:
+ * DEVICE pointer, K doubles.  The K sets share every read of the event store (HBM and shared memory): the value-only
+ * sweep is bound by that feed, so K values cost little more than one.
+ * pwa_hvp_cached_batch: hv[k] = H(theta) v[k], k < K, at the theta of the last pwa_nll_grad_for_hvp call (as
+ * pwa_hvp_cached).  v, hv: DEVICE pointers, K x P doubles.  The K directions share the propagators, B F and A_h.
+ * pwa_hessian: H[i][j] = d2 NLL / dtheta_i dtheta_j at theta, P x P doubles (DEVICE, row-major), through
+ * pwa_nll_grad_for_hvp(theta) and pwa_hvp_cached_batch on the unit vectors; replaces the kept state.  Its inverse on
+ * the free parameters is the covariance estimate behind Table 1's errors.
+ * All three enqueue on the handle's stream and do not synchronise; each result equals the corresponding single call to
+ * rounding (another summation tree).  K is split into the batch sizes the kernels are built for (values: 4 and 2,
+ * directions: 3 and 2); shapes served by the generic or the 8-event-tile kernel, and remainders of one, take one pass
+ * per evaluation.  The non-finite flag of pwa_status_flags refers to the last pass only.
+ * PWA_ERR_INVALID_ARG: K < 1, null pointers, pwa_hvp_cached_batch before any pwa_nll_grad_for_hvp. */
+pwa_status pwa_nll_batch(pwa_handle* h, int32_t K, const double* theta, double* nll);
+pwa_status pwa_hvp_cached_batch(pwa_handle* h, int32_t K, const double* v, double* hv);
+pwa_status pwa_hessian(pwa_handle* h, const double* theta, double* hess);
+
 /* ---- shard interface (Eqs. 4-7) -----------------------------------------------
  * pwa_raw_sums runs the same streaming pass but stops before the logarithm / division of Eqs. 4, 6, 7
  * and writes the ADDITIVE raw sums of this handle's events:  raw[pwa_raw_size(h)] doubles (device)

@@ -17,7 +17,7 @@ from typing import Optional
 __all__ = ["PwaError", "lib_path", "load", "pwa_create", "pwa_destroy", "pwa_n_params", "pwa_raw_size", "pwa_nll",
            "pwa_nll_grad", "pwa_hvp", "pwa_nll_grad_hvp", "pwa_raw_sums", "pwa_combine", "pwa_fit_opts",
            "pwa_fit_result", "pwa_fit_opts_default", "pwa_fit_newton_cg", "pwa_nll_grad_hvp_host", "pwa_fit_fractions",
-           "pwa_nll_grad_for_hvp", "pwa_hvp_cached",
+           "pwa_nll_grad_for_hvp", "pwa_hvp_cached", "pwa_nll_batch", "pwa_hvp_cached_batch", "pwa_hessian",
            "pwa_status_flags", "pwa_profile_enable", "pwa_profile_read", "pwa_kernel_launches", "pwa_bytes_per_eval",
            "pwa_kernel_variant", "pwa_last_error", "pwa_version", "Model", "STATUS_NAMES", "EXPORTS"]
 
@@ -32,7 +32,8 @@ PWA_MEM_HOST, PWA_MEM_DEVICE = 0, 1
 # every symbol include/pwa.h declares
 EXPORTS = ["pwa_create", "pwa_destroy", "pwa_n_params", "pwa_nll", "pwa_nll_grad", "pwa_hvp", "pwa_nll_grad_hvp",
            "pwa_raw_size", "pwa_raw_sums", "pwa_combine", "pwa_fit_opts_default", "pwa_fit_newton_cg",
-           "pwa_nll_grad_hvp_host", "pwa_fit_fractions", "pwa_nll_grad_for_hvp", "pwa_hvp_cached", "pwa_status_flags", "pwa_profile_enable", "pwa_profile_read",
+           "pwa_nll_grad_hvp_host", "pwa_fit_fractions", "pwa_nll_grad_for_hvp", "pwa_hvp_cached", "pwa_nll_batch", "pwa_hvp_cached_batch", "pwa_hessian",
+           "pwa_status_flags", "pwa_profile_enable", "pwa_profile_read",
            "pwa_kernel_launches", "pwa_bytes_per_eval", "pwa_kernel_variant", "pwa_last_error", "pwa_version"]
 
 
@@ -101,6 +102,9 @@ def load():
     lib.pwa_fit_fractions.argtypes = [vp, dp, dp]
     lib.pwa_nll_grad_for_hvp.argtypes = [vp, dp, dp, dp]
     lib.pwa_hvp_cached.argtypes = [vp, dp, dp]
+    lib.pwa_nll_batch.argtypes = [vp, c_int32, dp, dp]
+    lib.pwa_hvp_cached_batch.argtypes = [vp, c_int32, dp, dp]
+    lib.pwa_hessian.argtypes = [vp, dp, dp]
     lib.pwa_status_flags.argtypes = [vp, POINTER(c_uint32)]
     lib.pwa_profile_enable.argtypes = [vp, c_int32]
     lib.pwa_profile_read.argtypes = [vp, POINTER(c_double), POINTER(c_int64)]
@@ -264,6 +268,24 @@ def pwa_hvp_cached(h, v, hv) -> None:
     _check(load().pwa_hvp_cached(h, _dev_f64(v, P, "v"), _dev_f64(hv, P, "hv")), h)
 
 
+def pwa_nll_batch(h, K: int, theta, nll) -> None:
+    """nll[k] (device, K doubles) <- NLL(theta[k]) for the K parameter sets theta[K][P] (device), one pass per batch."""
+    P = pwa_n_params(h)
+    _check(load().pwa_nll_batch(h, K, _dev_f64(theta, K * P, "theta"), _dev_f64(nll, K, "nll")), h)
+
+
+def pwa_hvp_cached_batch(h, K: int, v, hv) -> None:
+    """hv[k] <- H(theta) v[k] for K directions v[K][P] at the theta of the last pwa_nll_grad_for_hvp call."""
+    P = pwa_n_params(h)
+    _check(load().pwa_hvp_cached_batch(h, K, _dev_f64(v, K * P, "v"), _dev_f64(hv, K * P, "hv")), h)
+
+
+def pwa_hessian(h, theta, hess) -> None:
+    """hess[P][P] (device) <- Hessian of the NLL at theta (device)."""
+    P = pwa_n_params(h)
+    _check(load().pwa_hessian(h, _dev_f64(theta, P, "theta"), _dev_f64(hess, P * P, "hess")), h)
+
+
 def pwa_fit_fractions(h, theta, frac) -> None:
     """frac[n_res] (device) <- fit fractions over the MC sample at theta (device)."""
     P = pwa_n_params(h)
@@ -366,6 +388,28 @@ class Model:
         with self._on():
             pwa_hvp_cached(self.h, self._d(v), self.hv_t)
             return self.hv_t.cpu().numpy().copy()
+
+    def nll_batch(self, thetas):
+        with self._on():
+            th = self._d(thetas)
+            K = th.shape[0]
+            out = self.torch.zeros(K, dtype=self.torch.float64, device=self.dev)
+            pwa_nll_batch(self.h, K, th, out)
+            return out.cpu().numpy()
+
+    def hvp_cached_batch(self, vs):
+        with self._on():
+            v = self._d(vs)
+            K = v.shape[0]
+            out = self.torch.zeros(K, self.P, dtype=self.torch.float64, device=self.dev)
+            pwa_hvp_cached_batch(self.h, K, v, out)
+            return out.cpu().numpy()
+
+    def hessian(self, theta):
+        with self._on():
+            out = self.torch.zeros(self.P, self.P, dtype=self.torch.float64, device=self.dev)
+            pwa_hessian(self.h, self._d(theta), out)
+            return out.cpu().numpy()
 
     def fit_fractions(self, theta):
         with self._on():

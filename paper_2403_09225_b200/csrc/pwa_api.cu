@@ -8,6 +8,7 @@
 
 #include "pwa_internal.h"
 #include "pwa_kernels.cuh"
+#include "pwa_batch.cuh"
 
 namespace {
 std::mutex g_err_mutex;
@@ -342,7 +343,7 @@ extern "C" pwa_status pwa_destroy(pwa_handle* h) {
   DeviceGuard guard(h->device);
   cudaStreamSynchronize(h->stream);
   for (void* p : h->owned) if (p) cudaFree(p);
-  void* dev[] = {h->d_ch, h->d_K, h->d_partial, h->d_sums, h->d_raw, h->d_flags, h->d_io, h->d_fit, h->d_pcache, h->d_theta_keep};
+  void* dev[] = {h->d_ch, h->d_K, h->d_partial, h->d_sums, h->d_raw, h->d_flags, h->d_io, h->d_fit, h->d_pcache, h->d_theta_keep, h->d_batch};
   for (void* p : dev) if (p) cudaFree(p);
   for (cudaEvent_t e : h->prof_events) cudaEventDestroy(e);
   if (h->h_pin) cudaFreeHost(h->h_pin);
@@ -487,6 +488,75 @@ extern "C" pwa_status pwa_hvp_cached(pwa_handle* h, const double* v, double* hv)
   DeviceGuard guard(h->device);
   if (!v || !hv) return set_error(h, PWA_ERR_INVALID_ARG, "pwa_hvp_cached: null pointer", cudaSuccess);
   return eval_hvp_kept(h, v, hv);
+}
+
+// ---- K evaluations per pass over the event store -----------------------------------
+// Greedy split of K into the batch counts the kernels are instantiated for; shapes without a batch kernel (and a
+// remainder of one) go through the single-evaluation sweep: same results, one pass each.
+extern "C" pwa_status pwa_nll_batch(pwa_handle* h, int32_t K, const double* theta, double* nll) {
+  if (!h) return PWA_ERR_INVALID_ARG;
+  DeviceGuard guard(h->device);
+  PWA_REQUIRE(h, K >= 1 && theta && nll, "pwa_nll_batch: K < 1 or null pointer");
+  const int P = h->n_par;
+  int k = 0;
+  unsigned bad = 0;
+  (void)bad;
+  while (k < K) {
+    const int left = K - k;
+    int kb = 1;
+    if (left >= 4 && batch_supported(h, BK_NLL, 4)) kb = 4;
+    else if (left >= 2 && batch_supported(h, BK_NLL, 2)) kb = 2;
+    pwa_status st = kb == 1 ? eval(h, MODE_NLL, theta + (size_t)k * P, nullptr, nll + k, nullptr, nullptr)
+                            : batch_launch(h, BK_NLL, kb, theta + (size_t)k * P, nullptr, nll + k);
+    if (st != PWA_OK) return st;
+    k += kb;
+  }
+  return PWA_OK;
+}
+
+extern "C" pwa_status pwa_hvp_cached_batch(pwa_handle* h, int32_t K, const double* v, double* hv) {
+  if (!h) return PWA_ERR_INVALID_ARG;
+  DeviceGuard guard(h->device);
+  PWA_REQUIRE(h, K >= 1 && v && hv, "pwa_hvp_cached_batch: K < 1 or null pointer");
+  if (!h->keep_valid) return set_error(h, PWA_ERR_INVALID_ARG, "pwa_hvp_cached_batch: no pwa_nll_grad_for_hvp call before", cudaSuccess);
+  const int P = h->n_par;
+  const int pref = std::getenv("PWA_HVP_BATCH") ? std::atoi(std::getenv("PWA_HVP_BATCH")) : 3;  // A/B runs
+  int k = 0;
+  while (k < K) {
+    const int left = K - k;
+    int kb = 1;
+    if (pref >= 3 && left >= 3 && batch_supported(h, BK_HVPQ, 3)) kb = 3;
+    else if (pref >= 2 && left >= 2 && batch_supported(h, BK_HVPQ, 2)) kb = 2;
+    pwa_status st = kb == 1 ? eval_hvp_kept(h, v + (size_t)k * P, hv + (size_t)k * P)
+                            : batch_launch(h, BK_HVPQ, kb, h->d_theta_keep, v + (size_t)k * P, hv + (size_t)k * P);
+    if (st != PWA_OK) return st;
+    k += kb;
+  }
+  return PWA_OK;
+}
+
+namespace {
+__global__ void k_identity(int P, double* V) {
+  for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < P * P; k += gridDim.x * blockDim.x) V[k] = (k / P == k % P) ? 1.0 : 0.0;
+}
+}  // namespace
+
+extern "C" pwa_status pwa_hessian(pwa_handle* h, const double* theta, double* hess) {
+  if (!h) return PWA_ERR_INVALID_ARG;
+  DeviceGuard guard(h->device);
+  PWA_REQUIRE(h, theta && hess, "pwa_hessian: null pointer");
+  const int P = h->n_par;
+  double* V = nullptr;
+  if (cudaMallocAsync(&V, sizeof(double) * P * P, h->stream) != cudaSuccess) {
+    cudaGetLastError();
+    return set_error(h, PWA_ERR_OOM, "pwa_hessian: scratch allocation failed", cudaSuccess);
+  }
+  k_identity<<<(P * P + 255) / 256, 256, 0, h->stream>>>(P, V);
+  h->launches++;
+  pwa_status st = eval_grad_keep(h, theta, h->d_io, h->d_io + 1);  // nll, grad into the staging area (not returned)
+  if (st == PWA_OK) st = pwa_hvp_cached_batch(h, P, V, hess);
+  cudaFreeAsync(V, h->stream);
+  return st;
 }
 
 extern "C" int64_t pwa_kernel_launches(const pwa_handle* h) { return h ? h->launches : -1; }

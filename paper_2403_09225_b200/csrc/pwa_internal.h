@@ -47,6 +47,8 @@ struct pwa_handle {
   double* d_io = nullptr;   // theta | v | nll | grad | hv   (1 + 4P doubles, padded)
   double* h_pin = nullptr;  // pinned host mirror of d_io
   double* d_fit = nullptr;  // fit vectors
+  double* d_batch = nullptr;       // batch sweeps: per-block partial rows, column sums, one raw vector
+  size_t batch_doubles = 0;
   double* h_fit = nullptr;  // pinned scalars of the fit driver
 
   long long launches = 0;
@@ -83,6 +85,16 @@ lanes_fn lanes_kernel_h2(int combo, int mode);
 lanes_fn lanes_kernel_h3(int combo, int mode);
 lanes_fn lanes_kernel_h4(int combo, int mode);
 lanes_fn lanes_kernel(int H, int combo, int mode);
+// batch kernels (pwa_batch.cuh): kind 0 = K parameter sets (value only), 1 = K directions at the kept theta
+struct BatchArgs;
+typedef void (*batch_fn)(const LaneArgs, const BatchArgs);
+batch_fn batch_kernel_h1(int rho, int log_sw, int kind, int kb);
+batch_fn batch_kernel_h2(int rho, int log_sw, int kind, int kb);
+batch_fn batch_kernel_h3(int rho, int log_sw, int kind, int kb);
+batch_fn batch_kernel_h4(int rho, int log_sw, int kind, int kb);
+// one batch pass of kb (a supported count) sets / directions: sweep + reduction; false if this handle's shape has no batch kernel
+bool batch_supported(const pwa_handle* h, int kind, int kb);
+pwa_status batch_launch(pwa_handle* h, int kind, int kb, const double* theta, const double* v, double* out);
 pwa_status lanes_configure(pwa_handle* h, std::string& why);  // sets variant = 2 on success; PWA_OK + why if unsuitable
 pwa_status lanes_launch(pwa_handle* h, int mode, const double* theta, const double* v, const double* skip = nullptr);
 // internal entry points used by the fit driver (enqueue only)

@@ -8,7 +8,7 @@ namespace pwa {
 // Prologue: per-resonance constants from theta (and v).  One thread per resonance.
 // PAPER.md:60 (couplings Lambda, here a e^{i phi}); BASELINE.json configs[0] (BW form).
 // ------------------------------------------------------------------------------------------------
-__global__ void k_prologue(const double* __restrict__ theta, const double* __restrict__ v, int R,
+static __global__ void k_prologue(const double* __restrict__ theta, const double* __restrict__ v, int R,
                            double* __restrict__ K) {
   int r = blockIdx.x * blockDim.x + threadIdx.x;
   if (r >= R) return;
@@ -342,7 +342,7 @@ __device__ __forceinline__ void combine_block(const double* raw, const double* _
   if (threadIdx.x == 0) *flags = bad ? 1u : 0u;
 }
 
-__global__ void __launch_bounds__(1024) k_combine(const double* raw, const double* __restrict__ v, int P,
+static __global__ void __launch_bounds__(1024) k_combine(const double* raw, const double* __restrict__ v, int P,
                                                   double* __restrict__ nll, double* __restrict__ grad,
                                                   double* __restrict__ hv, unsigned* __restrict__ flags) {
   combine_block(raw, v, P, nll, grad, hv, flags);

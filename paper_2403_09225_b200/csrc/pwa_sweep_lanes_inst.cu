@@ -1,6 +1,7 @@
 // pwa_sweep_lanes_inst.cu - instantiates the lanes sweep kernel for ONE helicity count (-DPWA_LANES_H=1..4), so that
 // the four counts compile in parallel (build.py).  The (RHO, LOG_SW, NW) table must match kLanesCombos in pwa_internal.h.
 #include "pwa_internal.h"
+#include "pwa_batch.cuh"
 
 #ifndef PWA_LANES_H
 #error "compile with -DPWA_LANES_H=<n_hel>"
@@ -38,6 +39,27 @@ lanes_fn PWA_CAT(lanes_kernel_h, PWA_LANES_H)(int combo, int mode) {
     case 11: return for_mode<4, 5, 8, 2, 8>(mode);
     case 12: return for_mode<4, 3, 11, 3>(mode);
   }
+  return nullptr;
+}
+
+// batch kernels (pwa_batch.cuh): only the warpgroup shapes (8 compute warps, 32-event tiles); kb: sets / directions per pass
+namespace {
+template <int RHO, int LOG_SW>
+batch_fn batch_for(int kind, int kb) {
+  if (kind == BK_NLL) {
+    if (kb == 2) return lanes::k_batch_lanes<PWA_LANES_H, RHO, LOG_SW, 8, BK_NLL, 2>;
+    if (kb == 4) return lanes::k_batch_lanes<PWA_LANES_H, RHO, LOG_SW, 8, BK_NLL, 4>;
+  } else {
+    if (kb == 2) return lanes::k_batch_lanes<PWA_LANES_H, RHO, LOG_SW, 8, BK_HVPQ, 2>;
+    if (kb == 3) return lanes::k_batch_lanes<PWA_LANES_H, RHO, LOG_SW, 8, BK_HVPQ, 3>;
+  }
+  return nullptr;
+}
+}  // namespace
+batch_fn PWA_CAT(batch_kernel_h, PWA_LANES_H)(int rho, int log_sw, int kind, int kb) {
+  if (rho == 3 && log_sw == 2) return batch_for<3, 2>(kind, kb);
+  if (rho == 4 && log_sw == 3) return batch_for<4, 3>(kind, kb);
+  // 16 or 32 slices (R > 32) leave fewer passes per tile than warps: no fixed column; those shapes take single passes
   return nullptr;
 }
 }  // namespace pwa
