@@ -84,7 +84,39 @@ typedef struct {
  * buffers), uploads or adopts the event store, allocates scratch.  *out is NULL on failure. */
 pwa_status pwa_create(const pwa_model_desc* model, pwa_handle** out);
 pwa_status pwa_destroy(pwa_handle* h); /* NULL is allowed */
-int32_t pwa_n_params(const pwa_handle* h); /* 4*n_res, or -1 for NULL */
+int32_t pwa_n_params(const pwa_handle* h); /* P: 4*n_res (2*n_res + 2*n_lineshape for a pwa_create_rich handle); -1 for NULL */
+
+/* ---- richer model: partial waves sharing resonance lineshapes, lineshape kinds (readings S21, S22) -------
+ * Eq. 1 sums partial-wave amplitudes Lambda_m U_m; a resonance contributes several partial waves
+ * ("phase angles and couplings of individual partial wave amplitudes") that share its mass and width
+ * (Table 1).  With a pwa_rich_desc the n_res plane groups of the model descriptor are PARTIAL WAVES m (coupling
+ * a_m e^{i phi_m}, planes F_mh); wave m takes its lineshape 1/D_l from resonance l = wave_res[m]:
+ *     A_h(i) = sum_m a_m e^{i phi_m} F_mh(i) / D_{wave_res[m]}(i)
+ * Lineshape kinds, m = mass[ls_chan[l]][i], parameters (M, Gamma) per resonance:
+ *   PWA_LS_CONST    D = M^2 - m^2 - i M Gamma                                                  (S4)
+ *   PWA_LS_MASSDEP  D = M^2 - m^2 - i M Gamma(m), Gamma(m) = Gamma (q(m)/q(M))^(2L+1) M/m, q = break-up momentum of
+ *                   (m1, m2); no barrier factors; shape = (m1, m2, L, -, -, -); needs M and every m above m1 + m2
+ *                   (else the result is NaN and the non-finite flag is raised)
+ *   PWA_LS_FLATTE   D = M^2 - m^2 - i Gamma (rho_1(m) + Rg rho_2(m)), rho_k = 2 q_k(m)/m for the channels (m1, m2) and
+ *                   (m3, m4), continued analytically below a threshold; "Gamma" is the coupling g_1, Rg = g_2/g_1
+ *                   fixed; shape = (m1, m2, m3, m4, Rg, -)
+ * Parameter layout of such a handle: theta = [a_0, phi_0, ..., a_{W-1}, phi_{W-1}, M_0, Gamma_0, ..., M_{L-1},
+ * Gamma_{L-1}], P = 2 n_res + 2 n_lineshape; every entry point (evaluation, raw sums, fit and its box, Hessian) uses
+ * it.  model->res_chan is ignored (channels come from ls_chan).  All arrays are HOST pointers, copied.
+ * Cost: models whose resonances are all PWA_LS_CONST run on the fast kernels (two extra tiny launches per evaluation
+ * expand theta, v and contract the sums: exact by the chain rule); a model with any other kind runs on the general-
+ * lineshape kernel (csrc/pwa_rich.cuh), which reads F twice per gradient / HVP evaluation.  pwa_fit_fractions returns
+ * per-WAVE fractions and supports PWA_LS_CONST only.  PWA_ERR_INVALID_ARG: n_lineshape not in [1, n_res], null
+ * arrays, wave_res / ls_chan / ls_kind out of range.  rich == NULL: same as pwa_create. */
+typedef enum { PWA_LS_CONST = 0, PWA_LS_MASSDEP = 1, PWA_LS_FLATTE = 2 } pwa_lineshape;
+typedef struct {
+  int32_t n_lineshape;      /* L resonances */
+  const int32_t* wave_res;  /* [n_res]       resonance of each partial wave, values in [0, L) */
+  const int32_t* ls_chan;   /* [L]           mass channel of each resonance */
+  const int32_t* ls_kind;   /* [L]           pwa_lineshape; NULL = all PWA_LS_CONST */
+  const double* ls_shape;   /* [L][6]        shape parameters per kind (above); may be NULL if every kind is CONST */
+} pwa_rich_desc;
+pwa_status pwa_create_rich(const pwa_model_desc* model, const pwa_rich_desc* rich, pwa_handle** out);
 
 /* ---- evaluation: device pointers, enqueue only ------------------------------------------------
  * theta, v, grad, hv: P doubles; nll: 1 double.  PAPER.md:67 (Eq. 3), :90 (Eq. 6), :95 (Eq. 7). */

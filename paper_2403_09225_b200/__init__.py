@@ -14,7 +14,7 @@ import os
 from ctypes import POINTER, Structure, byref, c_char_p, c_double, c_int32, c_int64, c_uint32, c_void_p
 from typing import Optional
 
-__all__ = ["PwaError", "lib_path", "load", "pwa_create", "pwa_destroy", "pwa_n_params", "pwa_raw_size", "pwa_nll",
+__all__ = ["PwaError", "lib_path", "load", "pwa_create", "pwa_create_rich", "pwa_rich_desc", "PWA_LS_CONST", "PWA_LS_MASSDEP", "PWA_LS_FLATTE", "pwa_destroy", "pwa_n_params", "pwa_raw_size", "pwa_nll",
            "pwa_nll_grad", "pwa_hvp", "pwa_nll_grad_hvp", "pwa_raw_sums", "pwa_combine", "pwa_fit_opts",
            "pwa_fit_result", "pwa_fit_opts_default", "pwa_fit_newton_cg", "pwa_nll_grad_hvp_host", "pwa_fit_fractions",
            "pwa_nll_grad_for_hvp", "pwa_hvp_cached", "pwa_nll_batch", "pwa_hvp_cached_batch", "pwa_hessian",
@@ -28,9 +28,10 @@ PWA_OK, PWA_ERR_INVALID_ARG, PWA_ERR_CUDA, PWA_ERR_OOM, PWA_ERR_NONFINITE, PWA_E
 STATUS_NAMES = ["PWA_OK", "PWA_ERR_INVALID_ARG", "PWA_ERR_CUDA", "PWA_ERR_OOM", "PWA_ERR_NONFINITE",
                 "PWA_ERR_NOT_CONVERGED"]
 PWA_MEM_HOST, PWA_MEM_DEVICE = 0, 1
+PWA_LS_CONST, PWA_LS_MASSDEP, PWA_LS_FLATTE = 0, 1, 2
 
 # every symbol include/pwa.h declares
-EXPORTS = ["pwa_create", "pwa_destroy", "pwa_n_params", "pwa_nll", "pwa_nll_grad", "pwa_hvp", "pwa_nll_grad_hvp",
+EXPORTS = ["pwa_create", "pwa_create_rich", "pwa_destroy", "pwa_n_params", "pwa_nll", "pwa_nll_grad", "pwa_hvp", "pwa_nll_grad_hvp",
            "pwa_raw_size", "pwa_raw_sums", "pwa_combine", "pwa_fit_opts_default", "pwa_fit_newton_cg",
            "pwa_nll_grad_hvp_host", "pwa_fit_fractions", "pwa_nll_grad_for_hvp", "pwa_hvp_cached", "pwa_nll_batch", "pwa_hvp_cached_batch", "pwa_hessian",
            "pwa_status_flags", "pwa_profile_enable", "pwa_profile_read",
@@ -52,6 +53,11 @@ class pwa_model_desc(Structure):
     _fields_ = [("n_res", c_int32), ("n_hel", c_int32), ("n_chan", c_int32), ("res_chan", c_void_p),
                 ("data", pwa_sample), ("mc", pwa_sample), ("mem", c_int32), ("borrow", c_int32),
                 ("device", c_int32), ("stream", c_void_p)]
+
+
+class pwa_rich_desc(Structure):
+    _fields_ = [("n_lineshape", c_int32), ("wave_res", c_void_p), ("ls_chan", c_void_p), ("ls_kind", c_void_p),
+                ("ls_shape", c_void_p)]
 
 
 class pwa_fit_opts(Structure):
@@ -86,6 +92,7 @@ def load():
     lib = ctypes.CDLL(path)
     vp, dp = c_void_p, c_void_p
     lib.pwa_create.argtypes = [POINTER(pwa_model_desc), POINTER(vp)]
+    lib.pwa_create_rich.argtypes = [POINTER(pwa_model_desc), POINTER(pwa_rich_desc), POINTER(vp)]
     lib.pwa_destroy.argtypes = [vp]
     lib.pwa_n_params.argtypes = [vp]
     lib.pwa_raw_size.argtypes = [vp]
@@ -149,11 +156,13 @@ def _dev_f64(t, n, name):
 # ---- the C calls, one to one ------------------------------------------------------------------------------
 def pwa_create(res_chan, data_mass, data_amp, data_weight, mc_mass, mc_amp, *, borrow: bool = False, device: int = 0,
                stream: int = 0, data_stride: int = 0, mc_stride: int = 0, n_data: Optional[int] = None,
-               n_mc: Optional[int] = None, data_first: int = 0, mc_first: int = 0) -> int:
+               n_mc: Optional[int] = None, data_first: int = 0, mc_first: int = 0, rich: Optional[dict] = None) -> int:
     """Creates a handle from torch tensors (CPU or CUDA, float64, contiguous) in the layouts of pwa.h:
     mass [C][N], amp [R][H][N][2], weight [N] or None, res_chan [R] int32 (CPU).  Returns the handle.
     A window of a larger store (an event shard) is described without copying by `*_first` (first
-    event), `n_*` (event count) and `*_stride` (events between planes of the full store)."""
+    event), `n_*` (event count) and `*_stride` (events between planes of the full store).
+    `rich` (pwa_create_rich, readings S21 / S22): dict with wave_res [R], ls_chan [L], and optionally ls_kind [L],
+    ls_shape [L][6]; res_chan is then ignored (may be None)."""
     import torch
     lib = load()
     tensors = [data_mass, data_amp, mc_mass, mc_amp] + ([data_weight] if data_weight is not None else [])
@@ -163,7 +172,7 @@ def pwa_create(res_chan, data_mass, data_amp, data_weight, mc_mass, mc_amp, *, b
     for t in tensors:
         if t.dtype != torch.float64 or not t.is_contiguous():
             raise TypeError("event buffers must be contiguous float64 tensors")
-    rc = res_chan.to(torch.int32).cpu().contiguous()
+    rc = (res_chan if res_chan is not None else torch.zeros(int(mc_amp.shape[0]))).to(torch.int32).cpu().contiguous()
     R, H = int(mc_amp.shape[0]), int(mc_amp.shape[1])
     C = int(mc_mass.shape[0])
     d = pwa_model_desc()
@@ -183,8 +192,31 @@ def pwa_create(res_chan, data_mass, data_amp, data_weight, mc_mass, mc_amp, *, b
     d.device = device
     d.stream = stream or None
     out = c_void_p()
-    _check(lib.pwa_create(byref(d), byref(out)))
+    if rich is None:
+        _check(lib.pwa_create(byref(d), byref(out)))
+        return out.value
+    i32 = lambda x: torch.as_tensor(x).to(torch.int32).cpu().contiguous()
+    wave_res, ls_chan = i32(rich["wave_res"]), i32(rich["ls_chan"])
+    if wave_res.numel() != R:
+        raise ValueError("rich['wave_res'] must have one entry per plane group (wave)")
+    L = int(ls_chan.numel())
+    kind = i32(rich["ls_kind"]) if rich.get("ls_kind") is not None else None
+    shape = (torch.as_tensor(rich["ls_shape"], dtype=torch.float64).cpu().contiguous()
+             if rich.get("ls_shape") is not None else None)
+    if kind is not None and kind.numel() != L:
+        raise ValueError("rich['ls_kind'] must have one entry per resonance")
+    if shape is not None and tuple(shape.shape) != (L, 6):
+        raise ValueError("rich['ls_shape'] must be [L][6]")
+    rd = pwa_rich_desc(L, wave_res.data_ptr(), ls_chan.data_ptr(), None if kind is None else kind.data_ptr(),
+                       None if shape is None else shape.data_ptr())
+    _check(lib.pwa_create_rich(byref(d), byref(rd), byref(out)))
     return out.value
+
+
+def pwa_create_rich(data_mass, data_amp, data_weight, mc_mass, mc_amp, rich: dict, **kw) -> int:
+    """pwa_create_rich of include/pwa.h: the plane groups are partial waves, `rich` maps them onto resonances
+    (wave_res, ls_chan, ls_kind, ls_shape); other keywords as pwa_create."""
+    return pwa_create(None, data_mass, data_amp, data_weight, mc_mass, mc_amp, rich=rich, **kw)
 
 
 def pwa_destroy(h) -> None:
@@ -289,7 +321,7 @@ def pwa_hessian(h, theta, hess) -> None:
 def pwa_fit_fractions(h, theta, frac) -> None:
     """frac[n_res] (device) <- fit fractions over the MC sample at theta (device)."""
     P = pwa_n_params(h)
-    _check(load().pwa_fit_fractions(h, _dev_f64(theta, P, "theta"), _dev_f64(frac, P // 4, "frac")), h)
+    _check(load().pwa_fit_fractions(h, _dev_f64(theta, P, "theta"), _dev_f64(frac, 1, "frac")), h)
 
 
 def pwa_status_flags(h) -> int:
@@ -334,7 +366,7 @@ class Model:
     """Owns a handle and its output tensors.  `w` is a workloads.Workload (or any object with the same fields).
     With `stream` (a cudaStream_t) the handle enqueues there, and so does every torch operation of this class."""
 
-    def __init__(self, w, device: int = 0, borrow: bool = False, stream: int = 0):
+    def __init__(self, w, device: int = 0, borrow: bool = False, stream: int = 0, rich: Optional[dict] = None):
         import contextlib
         import torch
         self.torch = torch
@@ -343,8 +375,9 @@ class Model:
         self._ext = torch.cuda.ExternalStream(stream, device=self.dev) if stream else None
         self._on = (lambda: torch.cuda.stream(self._ext)) if stream else contextlib.nullcontext
         self.h = pwa_create(w.res_chan, w.data_mass, w.data_amp, w.data_weight, w.mc_mass, w.mc_amp, borrow=borrow,
-                            device=device, stream=stream)
+                            device=device, stream=stream, rich=rich)
         self.P = pwa_n_params(self.h)
+        self._keep_R = int(w.mc_amp.shape[0])
         with self._on():
             self.nll_t = torch.zeros(1, dtype=torch.float64, device=self.dev)
             self.grad_t = torch.zeros(self.P, dtype=torch.float64, device=self.dev)
@@ -413,7 +446,7 @@ class Model:
 
     def fit_fractions(self, theta):
         with self._on():
-            frac = self.torch.zeros(self.P // 4, dtype=self.torch.float64, device=self.dev)
+            frac = self.torch.zeros(int(self._keep_R), dtype=self.torch.float64, device=self.dev)
             pwa_fit_fractions(self.h, self._d(theta), frac)
             return frac.cpu().numpy()
 

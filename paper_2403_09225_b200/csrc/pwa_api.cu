@@ -9,6 +9,7 @@
 #include "pwa_internal.h"
 #include "pwa_kernels.cuh"
 #include "pwa_batch.cuh"
+#include "pwa_rich.cuh"
 
 namespace {
 std::mutex g_err_mutex;
@@ -139,7 +140,118 @@ static pwa_status combine_impl(pwa_handle* h, const double* raw, const double* v
   return PWA_OK;
 }
 
+// ---- richer model (readings S21, S22): user vectors <-> the expanded space [n_res][4] the sweeps work in ----------
+// full[q] = user[map[q]] for theta (and v): exact, the expanded parameters are a linear (selection) map E of the user's
+static __global__ void k_expand(int n_full, const int* __restrict__ map, const double* __restrict__ theta,
+                                const double* __restrict__ v, double* __restrict__ theta_full, double* __restrict__ v_full) {
+  for (int q = blockIdx.x * blockDim.x + threadIdx.x; q < n_full; q += gridDim.x * blockDim.x) {
+    const int p = map[q];
+    if (theta) theta_full[q] = theta[p];
+    if (v) v_full[q] = v[p];
+  }
+}
+
+// raw_user = E^T raw_full block by block (every user parameter adds its expanded entries in ascending order), then -
+// with `combine` - Eqs. 4, 6, 7 on the user-sized vectors.  One block of 1024 threads.
+static __global__ void __launch_bounds__(1024) k_contract_combine(const double* __restrict__ raw_full, int n_full, int P,
+                                                                  const int* __restrict__ off, const int* __restrict__ idx,
+                                                                  double* raw, const double* __restrict__ v, int combine,
+                                                                  double* __restrict__ nll, double* __restrict__ grad,
+                                                                  double* __restrict__ hv, unsigned* __restrict__ flags) {
+  if (threadIdx.x < 4) raw[threadIdx.x] = raw_full[threadIdx.x];
+  for (int k = threadIdx.x; k < 4 * P; k += blockDim.x) {
+    const int blk = k / P, p = k - blk * P;
+    double t = 0.0;
+    for (int j = off[p]; j < off[p + 1]; ++j) t += raw_full[4 + (size_t)blk * n_full + idx[j]];
+    raw[4 + k] = t;
+  }
+  if (combine) {
+    __syncthreads();
+    combine_block(raw, v, P, nll, grad, hv, flags);
+  }
+}
+
+template <int MODE>
+static sweep_rich_fn rich_for_h(int H) {
+  switch (H) {
+    case 1: return k_sweep_rich<1, MODE>;
+    case 2: return k_sweep_rich<2, MODE>;
+    case 3: return k_sweep_rich<3, MODE>;
+    case 4: return k_sweep_rich<4, MODE>;
+  }
+  return nullptr;
+}
+
+// general-lineshape sweep (pwa_rich.cuh): prologue + sweep + reduction -> raw_full
+static pwa_status rich_raw(pwa_handle* h, int mode, const double* theta_full, const double* v_full, double* raw_full) {
+  const int W = h->n_res;
+  if (mode != MODE_NLL && mode != MODE_GRAD) mode = v_full ? MODE_FULL : MODE_GRAD;
+  double* K = h->d_full + 2 * (size_t)h->n_full + 4 + 4 * (size_t)h->n_full;
+  k_prologue_rich<<<(W + 127) / 128, 128, 0, h->stream>>>(theta_full, mode == MODE_FULL ? v_full : nullptr, W, h->d_wres,
+                                                         h->d_lkind, h->d_lshape, K);
+  h->launches++;
+  RichArgs a;
+  a.s[0] = h->smp[0];
+  a.s[1] = h->smp[1];
+  a.K = K;
+  a.wres = h->d_wres;
+  a.lch = h->d_lch;
+  a.lkind = h->d_lkind;
+  a.lshape = h->d_lshape;
+  a.W = W;
+  a.nb = (W + 3) / 4;
+  a.partial = h->d_partial;
+  sweep_rich_fn fn = mode == MODE_NLL ? rich_for_h<MODE_NLL>(h->n_hel) : mode == MODE_GRAD ? rich_for_h<MODE_GRAD>(h->n_hel) : rich_for_h<MODE_FULL>(h->n_hel);
+  if (!fn) return set_error(h, PWA_ERR_INVALID_ARG, "general-lineshape kernel: n_hel > 4", cudaSuccess);
+  const size_t smem = (size_t)(h->block / 32) * ((size_t)(mode == MODE_NLL ? 0 : a.nb * 32) + 2) * sizeof(double);
+  const bool prof = h->profiling && h->prof_used + 2 <= h->prof_events.size();
+  if (prof) cudaEventRecord(h->prof_events[h->prof_used], h->stream);
+  fn<<<h->grid, h->block, smem, h->stream>>>(a);
+  if (prof) {
+    cudaEventRecord(h->prof_events[h->prof_used + 1], h->stream);
+    h->prof_used += 2;
+  }
+  h->launches++;
+  if (cudaError_t ce = cudaGetLastError()) return set_error(h, PWA_ERR_CUDA, "launch k_sweep_rich", ce);
+  const double n_mc = (double)h->smp[0].n;
+  if (mode == MODE_NLL) k_reduce_rich<MODE_NLL><<<1, 1024, 0, h->stream>>>(h->d_partial, h->grid, a.nb, W, n_mc, h->d_sums, raw_full);
+  else k_reduce_rich<MODE_FULL><<<1, 1024, 0, h->stream>>>(h->d_partial, h->grid, a.nb, W, n_mc, h->d_sums, raw_full);
+  h->launches++;
+  if (cudaError_t ce = cudaGetLastError()) return set_error(h, PWA_ERR_CUDA, "launch k_reduce_rich", ce);
+  return PWA_OK;
+}
+
+// One evaluation of a pwa_create_rich handle.  theta == nullptr: the expanded theta kept in d_theta_keep is used
+// (split evaluation).  raw_user: where the contracted raw vector goes (h->d_raw or the caller's buffer).
+static pwa_status eval_mapped(pwa_handle* h, int mode, const double* theta, const double* v, double* raw_user, bool combine,
+                              double* nll, double* grad, double* hv, bool keep = false) {
+  const int nf = h->n_full;
+  double* th_full = (theta == nullptr || keep) ? h->d_theta_keep : h->d_full;
+  double* v_full = h->d_full + nf;
+  double* raw_full = h->d_full + 2 * (size_t)nf;
+  if (theta || v) {
+    k_expand<<<(nf + 255) / 256, 256, 0, h->stream>>>(nf, h->d_map, theta, v, th_full, v_full);
+    h->launches++;
+  }
+  pwa_status st = h->rich_kernel ? rich_raw(h, mode, th_full, v ? v_full : nullptr, raw_full)
+                                 : raw_sums_impl(h, mode, th_full, v ? v_full : nullptr, raw_full);
+  if (st != PWA_OK) return st;
+  k_contract_combine<<<1, 1024, 0, h->stream>>>(raw_full, nf, h->n_par, h->d_csr_off, h->d_csr_idx, raw_user, v, combine ? 1 : 0,
+                                                nll, grad, v ? hv : nullptr, h->d_flags);
+  h->launches++;
+  if (cudaError_t ce = cudaGetLastError()) return set_error(h, PWA_ERR_CUDA, "launch k_contract_combine", ce);
+  return PWA_OK;
+}
+
+pwa_status expand_theta(pwa_handle* h, const double* theta) {
+  k_expand<<<(h->n_full + 255) / 256, 256, 0, h->stream>>>(h->n_full, h->d_map, theta, nullptr, h->d_full, nullptr);
+  h->launches++;
+  if (cudaError_t ce = cudaGetLastError()) return set_error(h, PWA_ERR_CUDA, "launch k_expand", ce);
+  return PWA_OK;
+}
+
 pwa_status eval(pwa_handle* h, int mode, const double* theta, const double* v, double* nll, double* grad, double* hv) {
+  if (h->mapped) return eval_mapped(h, mode, theta, mode == MODE_FULL ? v : nullptr, h->d_raw, true, nll, grad, hv);
   // sweep, then ONE launch for the second reduction stage, the unpacking and Eqs. 4, 6, 7
   return raw_sums_impl(h, mode, theta, v, h->d_raw, true, nll, grad, hv);
 }
@@ -149,6 +261,12 @@ pwa_status eval(pwa_handle* h, int mode, const double* theta, const double* v, d
 // Shapes served by the generic kernel have no such modes: they fall back to the fused sweep at the kept theta.
 pwa_status eval_grad_keep(pwa_handle* h, const double* theta, double* nll, double* grad) {
   h->keep_valid = false;  // valid again only once everything that refreshes the kept state has been enqueued
+  if (h->mapped) {  // the kept theta is the expanded one
+    const int mode = (h->rich_kernel || h->variant < 2) ? MODE_GRAD : MODE_GRAD3;
+    const pwa_status stm = eval_mapped(h, mode, theta, nullptr, h->d_raw, true, nll, grad, nullptr, true);
+    h->keep_valid = stm == PWA_OK;
+    return stm;
+  }
   PWA_CUDA_CHECK(h, cudaMemcpyAsync(h->d_theta_keep, theta, sizeof(double) * h->n_par, cudaMemcpyDeviceToDevice, h->stream));
   const pwa_status st = h->variant < 2 ? eval(h, MODE_GRAD, theta, nullptr, nll, grad, nullptr)
                                        : raw_sums_impl(h, MODE_GRAD3, h->d_theta_keep, nullptr, h->d_raw, true, nll, grad, nullptr);
@@ -158,6 +276,10 @@ pwa_status eval_grad_keep(pwa_handle* h, const double* theta, double* nll, doubl
 
 pwa_status eval_hvp_kept(pwa_handle* h, const double* v, double* hv, const double* skip) {
   if (!h->keep_valid) return set_error(h, PWA_ERR_INVALID_ARG, "pwa_hvp_cached: no pwa_nll_grad_for_hvp call before", cudaSuccess);
+  if (h->mapped) {
+    const int mode = (h->rich_kernel || h->variant < 2) ? MODE_FULL : MODE_HVPQ;
+    return eval_mapped(h, mode, nullptr, v, h->d_raw, true, nullptr, nullptr, hv);
+  }
   if (h->variant < 2) return eval(h, MODE_FULL, h->d_theta_keep, v, nullptr, nullptr, hv);
   return raw_sums_impl(h, MODE_HVPQ, h->d_theta_keep, v, h->d_raw, true, nullptr, nullptr, hv, skip);
 }
@@ -226,16 +348,39 @@ static pwa_status store_sample(pwa_handle* h, const pwa_model_desc* m, const pwa
   return PWA_OK;
 }
 
-extern "C" pwa_status pwa_create(const pwa_model_desc* m, pwa_handle** out) {
+extern "C" pwa_status pwa_create(const pwa_model_desc* m, pwa_handle** out) { return pwa_create_rich(m, nullptr, out); }
+
+extern "C" pwa_status pwa_create_rich(const pwa_model_desc* m, const pwa_rich_desc* rich, pwa_handle** out) {
   if (out) *out = nullptr;
   if (!m || !out) return fail_create(nullptr, PWA_ERR_INVALID_ARG, "null descriptor or output pointer");
   if (m->n_res < 1 || m->n_res > PWA_MAX_RES) return fail_create(nullptr, PWA_ERR_INVALID_ARG, "n_res out of range");
   if (m->n_hel < 1 || m->n_hel > PWA_MAX_HEL) return fail_create(nullptr, PWA_ERR_INVALID_ARG, "n_hel out of range");
   if (m->n_chan < 1 || m->n_chan > PWA_MAX_CHAN) return fail_create(nullptr, PWA_ERR_INVALID_ARG, "n_chan out of range");
-  if (!m->res_chan) return fail_create(nullptr, PWA_ERR_INVALID_ARG, "null res_chan");
-  for (int r = 0; r < m->n_res; ++r)
-    if (m->res_chan[r] < 0 || m->res_chan[r] >= m->n_chan)
-      return fail_create(nullptr, PWA_ERR_INVALID_ARG, "res_chan value out of range");
+  std::vector<int> wave_chan(m->n_res);  // mass channel of every plane group (wave)
+  bool rich_kernel = false;
+  if (rich) {
+    if (rich->n_lineshape < 1 || rich->n_lineshape > m->n_res) return fail_create(nullptr, PWA_ERR_INVALID_ARG, "n_lineshape out of range");
+    if (!rich->wave_res || !rich->ls_chan) return fail_create(nullptr, PWA_ERR_INVALID_ARG, "null wave_res or ls_chan");
+    for (int l = 0; l < rich->n_lineshape; ++l) {
+      if (rich->ls_chan[l] < 0 || rich->ls_chan[l] >= m->n_chan) return fail_create(nullptr, PWA_ERR_INVALID_ARG, "ls_chan value out of range");
+      const int kind = rich->ls_kind ? rich->ls_kind[l] : PWA_LS_CONST;
+      if (kind < PWA_LS_CONST || kind > PWA_LS_FLATTE) return fail_create(nullptr, PWA_ERR_INVALID_ARG, "ls_kind value out of range");
+      if (kind != PWA_LS_CONST) rich_kernel = true;
+    }
+    if (rich_kernel && !rich->ls_shape) return fail_create(nullptr, PWA_ERR_INVALID_ARG, "null ls_shape with a non-constant-width resonance");
+    if (rich_kernel && m->n_hel > 4) return fail_create(nullptr, PWA_ERR_INVALID_ARG, "the general-lineshape kernel serves n_hel <= 4");
+    for (int w = 0; w < m->n_res; ++w) {
+      if (rich->wave_res[w] < 0 || rich->wave_res[w] >= rich->n_lineshape) return fail_create(nullptr, PWA_ERR_INVALID_ARG, "wave_res value out of range");
+      wave_chan[w] = rich->ls_chan[rich->wave_res[w]];
+    }
+  } else {
+    if (!m->res_chan) return fail_create(nullptr, PWA_ERR_INVALID_ARG, "null res_chan");
+    for (int r = 0; r < m->n_res; ++r) {
+      if (m->res_chan[r] < 0 || m->res_chan[r] >= m->n_chan)
+        return fail_create(nullptr, PWA_ERR_INVALID_ARG, "res_chan value out of range");
+      wave_chan[r] = m->res_chan[r];
+    }
+  }
   std::string why;
   if (!validate_sample(m->data, "data", why) || !validate_sample(m->mc, "mc", why))
     return fail_create(nullptr, PWA_ERR_INVALID_ARG, why);
@@ -264,7 +409,11 @@ extern "C" pwa_status pwa_create(const pwa_model_desc* m, pwa_handle** out) {
   h->n_res = m->n_res;
   h->n_hel = m->n_hel;
   h->n_chan = m->n_chan;
-  h->n_par = 4 * m->n_res;
+  h->n_full = 4 * m->n_res;
+  h->mapped = rich != nullptr;
+  h->rich_kernel = rich_kernel;
+  h->n_ls = rich ? rich->n_lineshape : m->n_res;
+  h->n_par = rich ? 2 * m->n_res + 2 * rich->n_lineshape : h->n_full;
   h->weighted = m->data.weight != nullptr;
   cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, m->device);
 
@@ -277,8 +426,8 @@ extern "C" pwa_status pwa_create(const pwa_model_desc* m, pwa_handle** out) {
   }
 
   // ---- launch configuration of the sweep (fixed for the life of the handle) ------------------------
-  const int R = h->n_res, P = h->n_par;
-  const int nb_full = nb_of(R, MODE_FULL);
+  const int R = h->n_res, P = h->n_full;  // scratch is sized for the expanded space
+  const int nb_full = std::max(nb_of(R, MODE_FULL), (R + 3) / 4);
   if (cudaMalloc(&h->d_ch, sizeof(int) * R) != cudaSuccess) {
     cudaGetLastError();
     return fail_create(h, PWA_ERR_OOM, "scratch allocation failed");
@@ -286,7 +435,7 @@ extern "C" pwa_status pwa_create(const pwa_model_desc* m, pwa_handle** out) {
   why.clear();
   h->weight_padded = h->owned[5] != nullptr;
   const char* force = std::getenv("PWA_VARIANT");
-  const bool want_lanes = !force || std::strcmp(force, "lanes") == 0;
+  const bool want_lanes = (!force || std::strcmp(force, "lanes") == 0) && !rich_kernel;
   if (want_lanes) {
     st = lanes_configure(h, why);
     if (st != PWA_OK) return fail_create(h, st, h->err);
@@ -310,6 +459,24 @@ extern "C" pwa_status pwa_create(const pwa_model_desc* m, pwa_handle** out) {
     h->block = block;
     h->grid = h->num_sms * occ_min;
     std::snprintf(h->variant_name, sizeof(h->variant_name), "generic(%s)", why.c_str());
+    if (rich_kernel) {
+      const size_t rsmem = (size_t)(block / 32) * ((size_t)((R + 3) / 4) * 32 + 2) * sizeof(double);
+      int occ_r = 1 << 30;
+      for (int mode = 0; mode < 3; ++mode) {
+        sweep_rich_fn fn = mode == MODE_NLL ? rich_for_h<MODE_NLL>(h->n_hel) : mode == MODE_GRAD ? rich_for_h<MODE_GRAD>(h->n_hel) : rich_for_h<MODE_FULL>(h->n_hel);
+        if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess)
+          return fail_create(h, PWA_ERR_CUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(ce));
+        int occ = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, block, mode == MODE_NLL ? (size_t)(block / 32) * 16 : rsmem);
+        occ_r = std::min(occ_r, std::max(occ, 1));
+      }
+      h->grid = h->num_sms * occ_r;
+      std::snprintf(h->variant_name, sizeof(h->variant_name), "rich(general lineshape, one thread per event)");
+    }
+  }
+  if (h->mapped && !rich_kernel) {
+    const size_t len = std::strlen(h->variant_name);
+    std::snprintf(h->variant_name + len, sizeof(h->variant_name) - len, "+shared");
   }
 
   const size_t pstride = std::max((size_t)nb_full * 32, (size_t)R * 10) + 2;
@@ -321,7 +488,7 @@ extern "C" pwa_status pwa_create(const pwa_model_desc* m, pwa_handle** out) {
             cudaMalloc(&h->d_raw, sizeof(double) * (4 + 4 * (size_t)P)) == cudaSuccess &&
             cudaMalloc(&h->d_flags, 2 * sizeof(unsigned)) == cudaSuccess &&
             cudaMalloc(&h->d_pcache, sizeof(double) * 2 * (6 * (size_t)h->n_res + 2)) == cudaSuccess &&
-            cudaMalloc(&h->d_theta_keep, sizeof(double) * h->n_par) == cudaSuccess &&
+            cudaMalloc(&h->d_theta_keep, sizeof(double) * h->n_full) == cudaSuccess &&
             cudaMalloc(&h->d_io, sizeof(double) * io) == cudaSuccess &&
             cudaMalloc(&h->d_fit, sizeof(double) * (8 * (size_t)P + 64)) == cudaSuccess &&
             cudaMallocHost(&h->h_pin, sizeof(double) * io) == cudaSuccess &&
@@ -330,7 +497,46 @@ extern "C" pwa_status pwa_create(const pwa_model_desc* m, pwa_handle** out) {
     cudaGetLastError();
     return fail_create(h, PWA_ERR_OOM, "scratch allocation failed");
   }
-  if ((ce = cudaMemcpyAsync(h->d_ch, m->res_chan, sizeof(int) * R, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
+  if (h->mapped) {
+    const int L = h->n_ls, nf = h->n_full, Pu = h->n_par;
+    std::vector<int> map(nf), off(Pu + 1, 0), idx(nf), kind(L, PWA_LS_CONST);
+    for (int w = 0; w < R; ++w) {
+      map[4 * w] = 2 * w;
+      map[4 * w + 1] = 2 * w + 1;
+      map[4 * w + 2] = 2 * R + 2 * rich->wave_res[w];
+      map[4 * w + 3] = 2 * R + 2 * rich->wave_res[w] + 1;
+    }
+    for (int q = 0; q < nf; ++q) off[map[q] + 1]++;
+    for (int p2 = 0; p2 < Pu; ++p2) off[p2 + 1] += off[p2];
+    {
+      std::vector<int> fill(off.begin(), off.end() - 1);
+      for (int q = 0; q < nf; ++q) idx[fill[map[q]]++] = q;  // ascending q within each user parameter
+    }
+    if (rich->ls_kind) kind.assign(rich->ls_kind, rich->ls_kind + L);
+    std::vector<double> shape((size_t)L * RICH_SP, 0.0);
+    if (rich->ls_shape) shape.assign(rich->ls_shape, rich->ls_shape + (size_t)L * RICH_SP);
+    const size_t full_doubles = 2 * (size_t)nf + 4 + 4 * (size_t)nf + (size_t)R * RK;
+    bool okr = cudaMalloc(&h->d_map, sizeof(int) * nf) == cudaSuccess && cudaMalloc(&h->d_csr_off, sizeof(int) * (Pu + 1)) == cudaSuccess &&
+               cudaMalloc(&h->d_csr_idx, sizeof(int) * nf) == cudaSuccess && cudaMalloc(&h->d_wres, sizeof(int) * R) == cudaSuccess &&
+               cudaMalloc(&h->d_lch, sizeof(int) * L) == cudaSuccess && cudaMalloc(&h->d_lkind, sizeof(int) * L) == cudaSuccess &&
+               cudaMalloc(&h->d_lshape, sizeof(double) * L * RICH_SP) == cudaSuccess &&
+               cudaMalloc(&h->d_full, sizeof(double) * full_doubles) == cudaSuccess;
+    if (!okr) {
+      cudaGetLastError();
+      return fail_create(h, PWA_ERR_OOM, "scratch allocation failed");
+    }
+    // pageable sources: cudaMemcpyAsync returns after staging them, the vectors may go out of scope
+    if ((ce = cudaMemcpyAsync(h->d_map, map.data(), sizeof(int) * nf, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
+        (ce = cudaMemcpyAsync(h->d_csr_off, off.data(), sizeof(int) * (Pu + 1), cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
+        (ce = cudaMemcpyAsync(h->d_csr_idx, idx.data(), sizeof(int) * nf, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
+        (ce = cudaMemcpyAsync(h->d_wres, rich->wave_res, sizeof(int) * R, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
+        (ce = cudaMemcpyAsync(h->d_lch, rich->ls_chan, sizeof(int) * L, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
+        (ce = cudaMemcpyAsync(h->d_lkind, kind.data(), sizeof(int) * L, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
+        (ce = cudaMemcpyAsync(h->d_lshape, shape.data(), sizeof(double) * L * RICH_SP, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
+        (ce = cudaStreamSynchronize(h->stream)) != cudaSuccess)
+      return fail_create(h, PWA_ERR_CUDA, std::string("upload: ") + cudaGetErrorString(ce));
+  }
+  if ((ce = cudaMemcpyAsync(h->d_ch, wave_chan.data(), sizeof(int) * R, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
       (ce = cudaMemsetAsync(h->d_flags, 0, 2 * sizeof(unsigned), h->stream)) != cudaSuccess ||
       (ce = cudaStreamSynchronize(h->stream)) != cudaSuccess)
     return fail_create(h, PWA_ERR_CUDA, std::string("upload: ") + cudaGetErrorString(ce));
@@ -343,7 +549,8 @@ extern "C" pwa_status pwa_destroy(pwa_handle* h) {
   DeviceGuard guard(h->device);
   cudaStreamSynchronize(h->stream);
   for (void* p : h->owned) if (p) cudaFree(p);
-  void* dev[] = {h->d_ch, h->d_K, h->d_partial, h->d_sums, h->d_raw, h->d_flags, h->d_io, h->d_fit, h->d_pcache, h->d_theta_keep, h->d_batch};
+  void* dev[] = {h->d_ch, h->d_K, h->d_partial, h->d_sums, h->d_raw, h->d_flags, h->d_io, h->d_fit, h->d_pcache, h->d_theta_keep, h->d_batch,
+                 h->d_map, h->d_csr_off, h->d_csr_idx, h->d_wres, h->d_lch, h->d_lkind, h->d_lshape, h->d_full};
   for (void* p : dev) if (p) cudaFree(p);
   for (cudaEvent_t e : h->prof_events) cudaEventDestroy(e);
   if (h->h_pin) cudaFreeHost(h->h_pin);
@@ -393,6 +600,7 @@ extern "C" pwa_status pwa_raw_sums(pwa_handle* h, const double* theta, const dou
   if (!h) return PWA_ERR_INVALID_ARG;
   DeviceGuard guard(h->device);
   PWA_REQUIRE(h, theta && raw, "pwa_raw_sums: null pointer");
+  if (h->mapped) return eval_mapped(h, v ? MODE_FULL : MODE_GRAD, theta, v, raw, false, nullptr, nullptr, nullptr);
   return raw_sums_impl(h, v ? MODE_FULL : MODE_GRAD, theta, v, raw);
 }
 

@@ -45,11 +45,12 @@ __device__ double block_max(double x, double* red) {
 // the box of reading S19: only M (k % 4 == 2) and Gamma (k % 4 == 3) are bounded; (0, 0) = no box
 struct Box {
   double gmin, gmax, mmin, mmax;
+  int split;  // < 0: interleaved (a, phi, M, Gamma) per resonance (S6); >= 0: [a, phi per wave | M, Gamma per resonance] (S21)
 };
 __device__ __forceinline__ void box_of(const Box& b, int k, double& lo, double& hi) {
   lo = -CUDART_INF;
   hi = CUDART_INF;
-  const int kind = k & 3;
+  const int kind = b.split < 0 ? (k & 3) : (k < b.split ? (k & 1) : 2 + ((k - b.split) & 1));
   if (kind == 2 && !(b.mmin == 0.0 && b.mmax == 0.0)) { lo = b.mmin; hi = b.mmax; }
   if (kind == 3 && !(b.gmin == 0.0 && b.gmax == 0.0)) { lo = b.gmin; hi = b.gmax; }
 }
@@ -215,7 +216,7 @@ extern "C" pwa_status pwa_fit_newton_cg(pwa_handle* h, double* theta, const pwa_
   double *g = h->d_fit, *z = g + P, *r = z + P, *d = r + P, *q = d + P, *p = q + P, *trial = p + P, *mask = trial + P,
          *sc = mask + P;
   double* hs = h->h_fit;
-  const Box box = {o.gamma_min, o.gamma_max, o.mass_min, o.mass_max};
+  const Box box = {o.gamma_min, o.gamma_max, o.mass_min, o.mass_max, h->mapped ? 2 * h->n_res : -1};
   auto fetch = [&]() -> cudaError_t {
     cudaError_t ce = cudaMemcpyAsync(hs, sc, sizeof(double) * S_N, cudaMemcpyDeviceToHost, st);
     if (ce != cudaSuccess) return ce;
@@ -259,7 +260,7 @@ extern "C" pwa_status pwa_fit_newton_cg(pwa_handle* h, double* theta, const pwa_
     // device-side status and return at once if CG has ended, so the host round trip hides behind the next sweep.
     // Shapes on the generic kernel have no such test and run one iteration at a time.
     bool have_p = false;
-    const bool pipelined = h->variant >= 2;
+    const bool pipelined = h->variant >= 2 && !h->mapped;
     int done_at = -1;
     double cg_end = 0.0;
     for (int j = 0; j < o.max_cg; ++j) {

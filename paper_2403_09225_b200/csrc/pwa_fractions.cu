@@ -116,6 +116,12 @@ extern "C" pwa_status pwa_fit_fractions(pwa_handle* h, const double* theta, doub
   if (!h) return PWA_ERR_INVALID_ARG;
   pwa::DeviceGuard guard(h->device);
   if (!theta || !frac) return set_error(h, PWA_ERR_INVALID_ARG, "pwa_fit_fractions: null pointer", cudaSuccess);
+  if (h->rich_kernel) return set_error(h, PWA_ERR_INVALID_ARG, "pwa_fit_fractions: constant-width resonances only", cudaSuccess);
+  if (h->mapped) {  // per-wave fractions at the expanded parameters
+    pwa_status st = pwa::expand_theta(h, theta);
+    if (st != PWA_OK) return st;
+    theta = h->d_full;
+  }
   frac_fn fn = frac_kernel(h->n_hel);
   if (!fn) return set_error(h, PWA_ERR_INVALID_ARG, "pwa_fit_fractions: n_hel out of range", cudaSuccess);
   const int R = h->n_res;

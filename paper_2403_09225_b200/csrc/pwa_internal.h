@@ -21,6 +21,21 @@ struct pwa_handle {
   void* owned[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
   int* d_ch = nullptr;
 
+  // richer model (readings S21, S22; pwa_create_rich): the kernels work in the EXPANDED parameter space [n_res][4]
+  // (every wave with its own a, phi, M, Gamma); user vectors are expanded before and contracted after a sweep
+  bool mapped = false;          // user parameter layout [a, phi per wave | M, Gamma per resonance]
+  bool rich_kernel = false;     // some resonance is not constant-width: k_sweep_rich (pwa_rich.cuh)
+  int n_full = 0;               // 4 * n_res
+  int n_ls = 0;                 // resonances (lineshapes)
+  int* d_map = nullptr;         // [n_full] expanded index -> user index
+  int* d_csr_off = nullptr;     // [n_par + 1] user parameter -> range in d_csr_idx
+  int* d_csr_idx = nullptr;     // [n_full] expanded indices, ascending within a user parameter
+  int* d_wres = nullptr;        // [n_res] resonance of each wave
+  int* d_lch = nullptr;         // [n_ls] channel of each resonance
+  int* d_lkind = nullptr;       // [n_ls]
+  double* d_lshape = nullptr;   // [n_ls][6]
+  double* d_full = nullptr;     // theta_full [n_full] | v_full [n_full] | raw_full [4 + 4 n_full] | K [n_res][16]
+
   // scratch
   double* d_K = nullptr;        // per-resonance constants
   double* d_partial = nullptr;  // per-block partial sums
@@ -103,6 +118,7 @@ pwa_status eval(pwa_handle* h, int mode, const double* theta, const double* v, d
 pwa_status eval_grad_keep(pwa_handle* h, const double* theta, double* nll, double* grad);
 pwa_status eval_hvp_kept(pwa_handle* h, const double* v, double* hv, const double* skip = nullptr);  // skip: LaneArgs::skip
 pwa_status set_error(pwa_handle* h, pwa_status st, const char* what, cudaError_t ce);
+pwa_status expand_theta(pwa_handle* h, const double* theta);  // rich handles: h->d_full[0 .. n_full) <- theta expanded
 }  // namespace pwa
 
 namespace pwa {

@@ -208,7 +208,7 @@ pwa_status lanes_launch(pwa_handle* h, int mode, const double* theta, const doub
 
 // ---- batch sweeps (pwa_batch.cuh) ---------------------------------------------------------------------------
 static batch_fn batch_kernel(const pwa_handle* h, int kind, int kb) {
-  if (h->variant < 2 || h->lanes_combo < 0) return nullptr;
+  if (h->variant < 2 || h->lanes_combo < 0 || h->mapped) return nullptr;  // rich handles take single passes
   const LanesCombo& c = kLanesCombos[h->lanes_combo];
   if (c.tile != 32) return nullptr;
   switch (h->n_hel) {
