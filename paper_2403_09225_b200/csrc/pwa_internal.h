@@ -93,7 +93,7 @@ struct LanesCombo {
 constexpr LanesCombo kLanesCombos[] = {
     {1, 2, 15, 0, 32, -1}, {2, 3, 15, 0, 32, -1}, {3, 2, 11, 0, 32, -1}, {3, 2, 8, 2, 32, -1}, {4, 3, 8, 2, 32, -1}, {4, 3, 7, 0, 32, -1},
     {4, 4, 8, 2, 32, -1},  {4, 4, 7, 0, 32, -1},  {4, 5, 8, 2, 32, -1},  {4, 5, 7, 0, 32, -1}, {4, 4, 8, 2, 8, -1},  {4, 5, 8, 2, 8, -1},
-    {4, 3, 11, 3, 32, -1}};
+    {4, 3, 11, 3, 32, -1}, {5, 1, 8, 2, 32, -1}};
 constexpr int kNumLanesCombos = sizeof(kLanesCombos) / sizeof(kLanesCombos[0]);
 lanes_fn lanes_kernel_h1(int combo, int mode);
 lanes_fn lanes_kernel_h2(int combo, int mode);

@@ -211,6 +211,7 @@ static batch_fn batch_kernel(const pwa_handle* h, int kind, int kb) {
   if (h->variant < 2 || h->lanes_combo < 0 || h->mapped) return nullptr;  // rich handles take single passes
   const LanesCombo& c = kLanesCombos[h->lanes_combo];
   if (c.tile != 32) return nullptr;
+  if (c.rho == 5 && kind == BK_HVPQ && kb == 3 && h->n_hel >= 3) return nullptr;  // spills (ptxas -v): batches of 2 there
   switch (h->n_hel) {
     case 1: return batch_kernel_h1(c.rho, c.log_sw, kind, kb);
     case 2: return batch_kernel_h2(c.rho, c.log_sw, kind, kb);

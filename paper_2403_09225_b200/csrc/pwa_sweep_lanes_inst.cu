@@ -38,6 +38,7 @@ lanes_fn PWA_CAT(lanes_kernel_h, PWA_LANES_H)(int combo, int mode) {
     case 10: return for_mode<4, 4, 8, 2, 8>(mode);
     case 11: return for_mode<4, 5, 8, 2, 8>(mode);
     case 12: return for_mode<4, 3, 11, 3>(mode);
+    case 13: return for_mode<5, 1, 8, 2>(mode);
   }
   return nullptr;
 }
@@ -57,6 +58,7 @@ batch_fn batch_for(int kind, int kb) {
 }
 }  // namespace
 batch_fn PWA_CAT(batch_kernel_h, PWA_LANES_H)(int rho, int log_sw, int kind, int kb) {
+  if (rho == 5 && log_sw == 1) return batch_for<5, 1>(kind, kb);
   if (rho == 3 && log_sw == 2) return batch_for<3, 2>(kind, kb);
   if (rho == 4 && log_sw == 3) return batch_for<4, 3>(kind, kb);
   // 16 or 32 slices (R > 32) leave fewer passes per tile than warps: no fixed column; those shapes take single passes

@@ -188,7 +188,8 @@ def test_zero_mass_resonance_on_a_ragged_tail(pwa, oracle_mod):
 
 
 @pytest.mark.parametrize("case,combo", [(CASES[2], 10), (CASES[2], 11), (CASES[1], 10), (CASES[0], 11), (CASES[4], 10),
-                                        (CASES[2], 5), (CASES[2], 6), (CASES[2], 12), (CASES[1], 3), (CASES[1], 1), (CASES[0], 0)])
+                                        (CASES[2], 5), (CASES[2], 6), (CASES[2], 12), (CASES[1], 3), (CASES[1], 1), (CASES[0], 0),
+                                        (CASES[1], 2), (CASES[1], 13), (CASES[4], 13)])
 def test_every_kernel_shape_matches_oracle(pwa, oracle_mod, case, combo, monkeypatch):
     """The handle normally picks one shape per (n_res, n_hel); PWA_COMBO forces another entry of kLanesCombos
     (csrc/pwa_internal.h) so that every instantiated shape - 8-event swizzled tiles, both producer kinds, every slice
