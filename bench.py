@@ -449,6 +449,14 @@ def main():
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms = float(t.item())
     nll_dev = m.nll_t.item()
+    ranks_agree = None
+    if world > 1:
+        # correctness anchor of the sharded path: after the all-reduce of the RAW sums every rank combines the same
+        # numbers, so the NLL (and with it theta along a fit) must be the same bits on every rank
+        allv = [torch.zeros(1, dtype=torch.float64, device=dev) for _ in range(world)]
+        dist.all_gather(allv, m.nll_t)
+        ranks_agree = all(x.item() == nll_dev for x in allv)
+        assert ranks_agree, "ranks disagree on the NLL after the all-reduce of the raw sums"
 
     # ---- end to end: H2D of theta, v (pinned) and D2H of nll, grad, hv every step, synchronised ----
     # one GPU: the library's host-buffer entry point; several: the same copies around raw sums -> all-reduce -> combine
@@ -545,7 +553,7 @@ def main():
                    "entry_point": MODES[args.mode],
                    "workload_gen_s": round(t_gen, 1)},
         "evals_per_s": evals_per_step * args.steps / (ms * 1e-3), "evals_per_step": evals_per_step,
-        "nll": nll_dev,
+        "nll": nll_dev, "nll_identical_across_ranks": ranks_agree,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": (achieved / peak) if achieved else None, "traffic": traffic,
                      "traffic_source": traffic_src, "peak_source": peak_src, "kernel": "sweep", "bytes_per_launch": bytes_per_step,
@@ -592,6 +600,8 @@ def main():
             reps += 1
         line["cpu_baseline"] = {"value": reps * (n_mc_s + n_data_s) / total, "unit": UNIT, "cores": threads,
                                 "kind": "oracle",
+                                "note": "the definitional oracle as it stands (gcc -O2, per-parameter derivatives, compensated "
+                                        "sums): a deliberately plain program, not a tuned CPU implementation",
                                 "sample": f"first {n_mc_s} MC + {n_data_s} data events of the same arrays, {reps} "
                                           f"NLL+grad+HVP evaluations ({total:.1f} s)",
                                 "nll_rel_diff_vs_gpu": abs(float(out[0]) - nll_dev) / max(abs(float(out[0])), 1.0)
