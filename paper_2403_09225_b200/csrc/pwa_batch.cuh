@@ -144,6 +144,22 @@ __global__ void __launch_bounds__(lanes_threads(NW, 2), 1) k_batch_lanes(const _
     const int r = j * SW + s;
     moff[j] = a.off_mass + (unsigned)(r < R ? a.ch[r] : 0) * (TILE * 8);
   }
+  // Constants in registers where the file has room (a shared load costs one wavefront per 4 bytes per lane, broadcast or
+  // not: the value batch of 4 spends 160 of its 240 wavefronts per pass on constants, its shared-memory pipe is 82 % busy;
+  // but 80 doubles of constants per lane cost more in lost instruction-level parallelism than they save).
+  constexpr int NKR = KIND == BK_NLL ? KB : 1;
+  constexpr bool KREG = KIND == BK_NLL && RHO * KB <= 8;  // measured: helps the batch of 2 (-5 %), hurts 4 sets and the direction batches
+  double2 k01r[RHO][NKR], cr[RHO][NKR];
+  double mgr[RHO][NKR];
+#pragma unroll
+  for (int j = 0; j < RHO; ++j)
+#pragma unroll
+    for (int k = 0; k < (KREG ? NKR : 0); ++k) {
+      const double2* kj = lane_k + j * (NSLOT * SW);
+      k01r[j][k] = kj[(3 * k) * SW];
+      mgr[j][k] = kj[(3 * k + 1) * SW].x;
+      cr[j][k] = kj[(3 * k + 2) * SW];
+    }
   // rows padded by 16 bytes: the EW event rows a warp reads back together start in different banks
   double* xrow = reinterpret_cast<double*>(smem_raw + b.off_xch) + ((size_t)w * EW + e) * (NV + 2);
 
@@ -179,9 +195,9 @@ __global__ void __launch_bounds__(lanes_threads(NW, 2), 1) k_batch_lanes(const _
         if (KIND == BK_NLL) {
 #pragma unroll
           for (int k = 0; k < KB; ++k) {
-            const double2 k01 = kj[(3 * k) * SW];
-            const double mg = kj[(3 * k + 1) * SW].x;
-            const double2 c = kj[(3 * k + 2) * SW];
+            const double2 k01 = KREG ? k01r[j][k] : kj[(3 * k) * SW];
+            const double mg = KREG ? mgr[j][k] : kj[(3 * k + 1) * SW].x;
+            const double2 c = KREG ? cr[j][k] : kj[(3 * k + 2) * SW];
             const double xx = fma(-m, m, k01.x);
             const double u = fast_rcp(fma(xx, xx, k01.y));
             const double br = xx * u, bi = mg * u;
@@ -199,9 +215,9 @@ __global__ void __launch_bounds__(lanes_threads(NW, 2), 1) k_batch_lanes(const _
             }
           }
         } else {
-          const double2 k01 = kj[0];
-          const double mg = kj[SW].x;
-          const double2 c = kj[2 * SW];
+          const double2 k01 = KREG ? k01r[j][0] : kj[0];
+          const double mg = KREG ? mgr[j][0] : kj[SW].x;
+          const double2 c = KREG ? cr[j][0] : kj[2 * SW];
           const double xx = fma(-m, m, k01.x);
           const double u = fast_rcp(fma(xx, xx, k01.y));
           const double br = xx * u, bi = mg * u;
