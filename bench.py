@@ -138,14 +138,14 @@ class ClockSampler:
 
 
 def _csrc_digest() -> str:
-    """sha256 over the kernel sources: ties a stored ncu traffic figure to the code it was captured on."""
+    """sha256 over the sources of the sweep kernel and its launch configuration: ties a stored ncu traffic figure to
+    the code it was captured on."""
     import hashlib
     d = os.path.join(ROOT, "paper_2403_09225_b200", "csrc")
     hsh = hashlib.sha256()
-    for name in sorted(os.listdir(d)):
-        if name.endswith((".cu", ".cuh", ".h")):
-            with open(os.path.join(d, name), "rb") as f:
-                hsh.update(name.encode() + b"\0" + f.read())
+    for name in ("pwa_common.cuh", "pwa_kernels.cuh", "pwa_sweep_lanes.cuh", "pwa_sweep_lanes.cu", "pwa_sweep_lanes_inst.cu"):
+        with open(os.path.join(d, name), "rb") as f:
+            hsh.update(name.encode() + b"\0" + f.read())
     return hsh.hexdigest()[:16]
 
 

@@ -119,7 +119,7 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
       off_mass = amp_bytes; off_wgt = up(off_mass + (unsigned)C * tile * 8, 128);  // TMA destinations: 128-byte aligned
       stage_bytes = up(off_wgt + tile * 8, tile == 32 ? 128 : 1024);
       k_bytes = up((unsigned)RP * lanes::KS * 8, 128);
-      xch_bytes = up((unsigned)NW * (32 / SW) * 4 * H * 8, 128);
+      xch_bytes = up((unsigned)NW * (32 / SW) * (4 * H + 2) * 8, 128);
       fixed = k_bytes + red_bytes + xch_bytes + 32u * 2 * 8 + 128;
       const int fit = (int)std::min<long long>(32, ((long long)dev_smem - fixed) / stage_bytes);
       stages = std::min(8, fit);  // deeper rings were measured no faster (the kernel is not feed-bound); PWA_STAGES overrides

@@ -41,7 +41,7 @@ struct alignas(64) LaneArgs {
   int R, C, stages;
   int nbox, rows_box;                       // amplitude rows are loaded in nbox boxes of rows_box rows (<= 256)
   unsigned stage_bytes, amp_bytes, off_mass, off_wgt;  // inside a stage: amplitude planes [rows][32 events], mass, weights
-  unsigned off_K, off_red, off_bar, off_xch;  // after the stages; xch: [NW][32/SW events][4H] doubles
+  unsigned off_K, off_red, off_bar, off_xch;  // after the stages; xch: [NW][32/SW events][4H + 2] doubles
 };
 
 namespace lanes {
@@ -368,7 +368,9 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
       creg[j] = kk[2];
     }
   }
-  double* xrow = reinterpret_cast<double*>(smem_raw + a.off_xch) + ((size_t)w * EW + e) * (4 * H);  // this event's exchange row
+  // this event's exchange row; rows are 4H + 2 doubles apart so that the EW rows a warp reads back together start in
+  // different banks (at 4H doubles the read-back of H = 2 had a 2-way conflict: 8 wavefronts per load instead of 4)
+  double* xrow = reinterpret_cast<double*>(smem_raw + a.off_xch) + ((size_t)w * EW + e) * (4 * H + 2);
 
   // pass g = w + k NW  ->  local tile t = g / NP, column col = g % NP.  When NW is a multiple of NP a warp keeps
   // its column for the whole sweep (FIXCOL): the event index, the amplitude and mass offsets inside a stage are then
