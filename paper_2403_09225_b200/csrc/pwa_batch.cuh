@@ -50,6 +50,9 @@ __global__ void __launch_bounds__(lanes_threads(NW, 2), 1) k_batch_lanes(const _
   constexpr int NACC = KIND == BK_NLL ? 0 : 4 * KB;  // per own resonance: Q1, Q2 of every direction
   constexpr int NA = NACC > 0 ? NACC : 1;
   constexpr int NS0 = KIND == BK_NLL ? KB : 1;
+  // PAIR (value batch, 8 slices x 4 events): a warp takes TWO columns of every second tile and a lane two events, one per
+  // column, odd slices in the opposite order - see the compute section
+  constexpr bool PAIR = KIND == BK_NLL && LOG_SW == 3 && NW == NP && KB >= 4;
   static_assert(NW % NP == 0, "a warp keeps its column");
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   const int lane = threadIdx.x & 31, w = (int)(threadIdx.x >> 5) - 4;  // w: compute-warp index (warps 0..3: producer group)
@@ -87,7 +90,7 @@ __global__ void __launch_bounds__(lanes_threads(NW, 2), 1) k_batch_lanes(const _
   if (threadIdx.x == 0) {
     for (int k = 0; k < stages; ++k) {
       mbar_init(full0 + 8 * k, 1);
-      mbar_init(empty0 + 8 * k, NP);
+      mbar_init(empty0 + 8 * k, PAIR ? NP / 2 : NP);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -162,6 +165,133 @@ __global__ void __launch_bounds__(lanes_threads(NW, 2), 1) k_batch_lanes(const _
     }
   // rows padded by 16 bytes: the EW event rows a warp reads back together start in different banks
   double* xrow = reinterpret_cast<double*>(smem_raw + b.off_xch) + ((size_t)w * EW + e) * (NV + 2);
+
+  if constexpr (PAIR) {
+    // ---- value batch, two events per lane -----------------------------------------------------------------------
+    // Warp w takes the column pair cp = w % 4 of the local tiles w / 4, w / 4 + 2, ...  A lane evaluates its RHO x KB
+    // propagators for TWO events: even slices first column 2cp then 2cp + 1, odd slices the other way round.  Then
+    //   - the constants of a (resonance, set) are read once for two events;
+    //   - a quarter-warp (two slices x four events) reads 128 CONTIGUOUS bytes of a plane row: no bank conflict
+    //     (with one column per warp the two slices hit the same banks);
+    //   - the first exchange level needs no selects: both lanes of a slice pair keep their first event and send the second;
+    //   - the event stage (I, ln I) runs once per event and slice pair instead of once per slice.
+    constexpr int NPP = NP / 2;
+    const int cp = w % NPP;
+    const int colA = 2 * cp + (s & 1), colB = 2 * cp + ((s & 1) ^ 1);
+    const int evA = colA * EW + e, evB = colB * EW + e;
+    double* xrowp = reinterpret_cast<double*>(smem_raw + b.off_xch) + ((size_t)w * EW + e) * (NV + 2) +
+                    (size_t)(s & 1) * ((size_t)NW * EW * (NV + 2));  // second half of the buffer: odd slices' events
+    int t = w / NPP;
+    for (int smp = 0; smp < 2; ++smp) {
+      const int t_end = smp ? T : TmB;
+      const int n = (int)(smp ? nD : nM);
+      const bool weighted = smp == 1 && a.weighted;
+#pragma unroll 1
+      while (t < t_end) {
+        const int st = t % stages, ph = (t / stages) & 1;
+        const int i0 = (bk + (t - (smp ? TmB : 0)) * G) * TILE;
+        const bool valid = i0 + evA < n;
+        mbar_wait(full0 + 8 * st, (uint32_t)ph);
+        const unsigned char* sp = smem_raw + (size_t)st * a.stage_bytes;
+        const unsigned char* fpA = sp + (unsigned)s * (H * TILE * 16) + evA * 16;
+        const unsigned char* fpB = sp + (unsigned)s * (H * TILE * 16) + evB * 16;
+        double wt = 1.0;
+        if (weighted) wt = reinterpret_cast<const double*>(sp + a.off_wgt)[evA];
+        double xa[NV], xb[NV];
+#pragma unroll
+        for (int j = 0; j < RHO; ++j) {
+          const double2* kj = lane_k + j * (NSLOT * SW);
+          const double mA = *reinterpret_cast<const double*>(sp + moff[j] + evA * 8);
+          const double mB = *reinterpret_cast<const double*>(sp + moff[j] + evB * 8);
+          double2 FA[H], FB[H];
+#pragma unroll
+          for (int h = 0; h < H; ++h) {
+            FA[h] = *reinterpret_cast<const double2*>(fpA + (j * SW * H + h) * (TILE * 16));
+            FB[h] = *reinterpret_cast<const double2*>(fpB + (j * SW * H + h) * (TILE * 16));
+          }
+#pragma unroll
+          for (int k = 0; k < KB; ++k) {
+            const double2 k01 = kj[(3 * k) * SW];
+            const double mg = kj[(3 * k + 1) * SW].x;
+            const double2 c = kj[(3 * k + 2) * SW];
+#pragma unroll
+            for (int side = 0; side < 2; ++side) {
+              const double m = side ? mB : mA;
+              const double xx = fma(-m, m, k01.x);
+              const double u = fast_rcp(fma(xx, xx, k01.y));
+              const double br = xx * u, bi = mg * u;
+              const double zr = fma(c.x, br, -(c.y * bi)), zi = fma(c.x, bi, c.y * br);
+#pragma unroll
+              for (int h = 0; h < H; ++h) {
+                const double2 F = side ? FB[h] : FA[h];
+                double* xk = (side ? xb : xa) + 2 * H * k + 2 * h;
+                if (j == 0) {
+                  xk[0] = fma(zr, F.x, -(zi * F.y));
+                  xk[1] = fma(zr, F.y, zi * F.x);
+                } else {
+                  xk[0] = fma(zr, F.x, fma(-zi, F.y, xk[0]));
+                  xk[1] = fma(zr, F.y, fma(zi, F.x, xk[1]));
+                }
+              }
+            }
+          }
+        }
+        __syncwarp();
+        mbar_arrive_if_zero(empty0 + 8 * st, (uint32_t)lane);
+        // exchange: level 1 over the slice pair (keep the first event, send the second), then the usual reduce-scatter
+        // over the remaining slice bits; every lane ends with its share of the totals of ITS first event
+#pragma unroll
+        for (int i = 0; i < NV; ++i) xa[i] += shfl_x(xb[i], EW);
+        slice_reduce_store<NV, 2 * EW>(xa, lane, xrowp);
+        __syncwarp();
+#pragma unroll
+        for (int i = 0; i < NV; i += 2) {
+          const double2 pr = *reinterpret_cast<const double2*>(xrowp + i);
+          xa[i] = pr.x;
+          xa[i + 1] = pr.y;
+        }
+        __syncwarp();
+        const double wv = valid ? wt : 0.0;
+#pragma unroll
+        for (int k = 0; k < KB; ++k) {
+          double I = 0.0;
+#pragma unroll
+          for (int h = 0; h < H; ++h) {
+            const double* xk = xa + 2 * H * k + 2 * h;
+            I = fma(xk[0], xk[0], fma(xk[1], xk[1], I));
+          }
+          if (smp == 0) s0[k] += I;
+          else s0[k] = fma(wv, log(valid ? I : 1.0), s0[k]);
+        }
+        if (smp == 1) s1 += wv;
+        t += NW / NPP;
+      }
+      // end of a sample: the lanes of slices 0 and 1 (lane < 2 EW) hold every event of the warp's columns once
+      double* out = b.partial + ((size_t)smp * gridDim.x + blockIdx.x) * (size_t)row_len;
+      double* mine = red + (size_t)w * row_len;
+#pragma unroll
+      for (int k = 0; k < KB; ++k) {
+        double t0 = s0[k];
+#pragma unroll
+        for (int m = 1; m < 2 * EW; m <<= 1) t0 += shfl_x(t0, m);
+        if (lane == 0) mine[k] = t0;
+        s0[k] = 0.0;
+      }
+      double t1 = s1;
+#pragma unroll
+      for (int m = 1; m < 2 * EW; m <<= 1) t1 += shfl_x(t1, m);
+      if (lane == 0) mine[KB] = t1;
+      s1 = 0.0;
+      asm volatile("bar.sync 1, %0;" ::"n"(NW * 32) : "memory");
+      for (int k = w * 32 + lane; k < row_len; k += NW * 32) {
+        double tsum = red[k];
+        for (int ww = 1; ww < NW; ++ww) tsum += red[(size_t)ww * row_len + k];
+        out[k] = tsum;
+      }
+      asm volatile("bar.sync 1, %0;" ::"n"(NW * 32) : "memory");
+    }
+    return;
+  }
 
   const int col = w % NP;
   int t = w / NP;

@@ -330,3 +330,30 @@ def test_unconstrained_parameter_domain(pwa, oracle_mod, idx, n_mc, n_data):
         if name == "a_1 = 0":
             assert g[4] != 0.0 and np.isfinite(g[4])
             assert abs(g[4] - float(g0[4])) <= 1e-8 * abs(float(g0[4]))
+
+
+def test_handle_used_from_another_host_thread(pwa, oracle_mod):
+    """PAPER.md:98 runs one host thread per GPU.  Every C-ABI entry binds the calling thread to the handle's device for
+    the duration of the call and restores the caller's current device (csrc/pwa_internal.h: DeviceGuard), so a handle
+    created in one thread gives the same bits when it is called from a fresh thread (whose CUDA context state is the
+    default one), and the caller's current device is left as it was.  (This pool has one GPU per box: the case of a
+    thread whose current device is ANOTHER ordinal cannot be run here.)"""
+    import threading
+    import workloads
+    cfg, w, om, gm = _case(pwa, oracle_mod, *CASES[1])
+    th = _thetas(cfg)[1]
+    v = workloads.direction(cfg, 3).numpy()
+    want = gm.nll_grad_hvp(th, v)
+    out = {}
+
+    def work():
+        before = torch.cuda.current_device()
+        out["res"] = gm.nll_grad_hvp(th, v)
+        out["fit"] = gm.fit(th, None)[1].status
+        out["dev"] = (before, torch.cuda.current_device())
+
+    t = threading.Thread(target=work)
+    t.start()
+    t.join()
+    assert out["res"][0] == want[0] and out["res"][1].tobytes() == want[1].tobytes() and out["res"][2].tobytes() == want[2].tobytes()
+    assert out["dev"][0] == out["dev"][1] and out["fit"] in (0, 5)

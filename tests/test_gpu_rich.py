@@ -181,3 +181,40 @@ def test_fit_of_a_shared_resonance_model(oracle_mod, env):
     assert np.all(th2[2 * W + 1::2] <= o2.gamma_max) and res2.n_active >= 1 and res2.nll > res.nll
     assert np.any(th2[0:2 * W:2] > o2.gamma_max)   # couplings are not boxed
     gm.close()
+
+
+def test_fit_runs_on_the_general_lineshape_kernel(oracle_mod, env):
+    """A few Newton-CG iterations on the mixed-kind model (k_sweep_rich serves value, gradient and HVP of the driver):
+    the NLL goes down, the reported value is the rich oracle's NLL at the returned point, the box holds."""
+    pwa, rich = env
+    rm, gm = _mixed(env, oracle_mod)
+    th0 = _theta(11, rm.n_wave, rm.n_ls)
+    o = pwa.pwa_fit_opts_default()
+    o.max_outer = 6
+    th, res = gm.fit(th0, o)
+    f_start = float(rich.nll(rm, th0, "d", threads=oracle_mod.max_threads()))
+    f_end = float(rich.nll(rm, th, "d", threads=oracle_mod.max_threads()))
+    assert res.outer_iters == 6 and res.stop_reason == 4 and res.n_hvp >= 6
+    assert res.nll < f_start and abs(res.nll - f_end) <= 1e-10 * max(1.0, abs(f_end))
+    W = rm.n_wave
+    assert np.all(th[2 * W::2] >= o.mass_min) and np.all(th[2 * W + 1::2] >= o.gamma_min)
+    gm.close()
+
+
+def test_per_wave_fractions_of_a_shared_resonance_model(oracle_mod, env):
+    """pwa_fit_fractions on a pwa_create_rich handle (constant widths): per-WAVE fractions at the expanded parameters,
+    against oracle/fractions.py on the base model the expansion defines."""
+    from oracle.fractions import fit_fractions
+    pwa, rich = env
+    rm, gm = _shared_const(env, oracle_mod)
+    th = _theta(4, rm.n_wave, rm.n_ls)
+    W = rm.n_wave
+    full = np.empty(4 * W)
+    full[0::4], full[1::4] = th[0:2 * W:2], th[1:2 * W:2]
+    full[2::4], full[3::4] = th[2 * W + 2 * rm.wave_res], th[2 * W + 2 * rm.wave_res + 1]
+    base = oracle_mod.Model(rm.res_chan[rm.wave_res], rm.data, rm.mc)
+    want = fit_fractions(base, full)
+    got = gm.fit_fractions(th)
+    assert got.shape == (W,)
+    assert np.max(np.abs(got - want)) <= 1e-10 * np.max(np.abs(want))
+    gm.close()
