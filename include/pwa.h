@@ -106,7 +106,7 @@ int32_t pwa_n_params(const pwa_handle* h); /* P: 4*n_res (2*n_res + 2*n_lineshap
  * Cost: models whose resonances are all PWA_LS_CONST run on the fast kernels (two extra tiny launches per evaluation
  * expand theta, v and contract the sums: exact by the chain rule); a model with any other kind runs on the general-
  * lineshape kernel (csrc/pwa_rich.cuh), which reads F twice per gradient / HVP evaluation.  pwa_fit_fractions returns
- * per-WAVE fractions and supports PWA_LS_CONST only.  PWA_ERR_INVALID_ARG: n_lineshape not in [1, n_res], null
+ * one fraction per RESONANCE (n_lineshape doubles): the coherent sum of its partial waves, any lineshape kind.  PWA_ERR_INVALID_ARG: n_lineshape not in [1, n_res], null
  * arrays, wave_res / ls_chan / ls_kind out of range.  rich == NULL: same as pwa_create. */
 typedef enum { PWA_LS_CONST = 0, PWA_LS_MASSDEP = 1, PWA_LS_FLATTE = 2 } pwa_lineshape;
 typedef struct {
@@ -224,7 +224,8 @@ pwa_status pwa_nll_grad_hvp_host(pwa_handle* h, const double* theta_host, const 
 
 /* ---- fit fractions (Table 1 of the paper lists a "fraction" F_i per resonance; S20) ----
  * frac[r] = sum_mc sum_h |c_r B_r(j) F_rh(j)|^2 / sum_mc I_j  over the handle's phase-space MC sample.
- * theta: DEVICE pointer, P doubles; frac: DEVICE pointer, n_res doubles.  Enqueues on the handle's stream (one pass
+ * pwa_create_rich handles: frac[l] = sum_mc sum_h |sum_{m in l} z_m(j) F_mh(j)|^2 / sum_mc I_j per resonance l.
+ * theta: DEVICE pointer, P doubles; frac: DEVICE pointer, n_res (rich handles: n_lineshape) doubles.  Enqueues on the handle's stream (one pass
  * over the MC event store), does not synchronise.  PWA_ERR_INVALID_ARG on null pointers. */
 pwa_status pwa_fit_fractions(pwa_handle* h, const double* theta, double* frac);
 

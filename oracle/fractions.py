@@ -38,3 +38,23 @@ def fit_fractions(model, theta) -> np.ndarray:
             own[r] += np.sum(t.real * t.real + t.imag * t.imag)
     total = np.sum(A.real * A.real + A.imag * A.imag)
     return np.asarray(own / total, dtype=np.float64)
+
+
+def fit_fractions_rich(model, theta) -> np.ndarray:
+    """Richer model (oracle/rich.py; S20, S21): one fraction per RESONANCE l, the coherent sum of its partial
+    waves,  F_l = sum_j sum_h | sum_{m in l} z_m(j) F_mh(j) |^2 / sum_j I_j.  Written as the definition says it: the
+    numerator is the MC intensity sum with every coupling outside resonance l switched off.  model: oracle.rich.RichModel;
+    theta in its [waves | resonances] layout.  Returns F[L] (float64)."""
+    from . import rich
+    ld = np.longdouble
+    th = np.asarray(theta, dtype=ld)
+    W, L = model.n_wave, model.n_ls
+    total = np.sum(np.asarray(rich.intensity(model, "mc", th, "ld"), dtype=ld))
+    out = np.zeros(L, dtype=ld)
+    for l in range(L):
+        only = th.copy()
+        for m in range(W):
+            if int(model.wave_res[m]) != l:
+                only[2 * m] = 0
+        out[l] = np.sum(np.asarray(rich.intensity(model, "mc", only, "ld"), dtype=ld)) / total
+    return np.asarray(out, dtype=np.float64)

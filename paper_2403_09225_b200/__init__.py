@@ -377,7 +377,7 @@ class Model:
         self.h = pwa_create(w.res_chan, w.data_mass, w.data_amp, w.data_weight, w.mc_mass, w.mc_amp, borrow=borrow,
                             device=device, stream=stream, rich=rich)
         self.P = pwa_n_params(self.h)
-        self._keep_R = int(w.mc_amp.shape[0])
+        self._keep_R = int(w.mc_amp.shape[0]) if rich is None else int(len(rich["ls_chan"]))  # fractions returned
         with self._on():
             self.nll_t = torch.zeros(1, dtype=torch.float64, device=self.dev)
             self.grad_t = torch.zeros(self.P, dtype=torch.float64, device=self.dev)

@@ -515,11 +515,19 @@ extern "C" pwa_status pwa_create_rich(const pwa_model_desc* m, const pwa_rich_de
     if (rich->ls_kind) kind.assign(rich->ls_kind, rich->ls_kind + L);
     std::vector<double> shape((size_t)L * RICH_SP, 0.0);
     if (rich->ls_shape) shape.assign(rich->ls_shape, rich->ls_shape + (size_t)L * RICH_SP);
+    std::vector<int> wl_off(L + 1, 0), wl_idx(R);
+    for (int w = 0; w < R; ++w) wl_off[rich->wave_res[w] + 1]++;
+    for (int l = 0; l < L; ++l) wl_off[l + 1] += wl_off[l];
+    {
+      std::vector<int> fill(wl_off.begin(), wl_off.end() - 1);
+      for (int w = 0; w < R; ++w) wl_idx[fill[rich->wave_res[w]]++] = w;
+    }
     const size_t full_doubles = 2 * (size_t)nf + 4 + 4 * (size_t)nf + (size_t)R * RK;
     bool okr = cudaMalloc(&h->d_map, sizeof(int) * nf) == cudaSuccess && cudaMalloc(&h->d_csr_off, sizeof(int) * (Pu + 1)) == cudaSuccess &&
                cudaMalloc(&h->d_csr_idx, sizeof(int) * nf) == cudaSuccess && cudaMalloc(&h->d_wres, sizeof(int) * R) == cudaSuccess &&
                cudaMalloc(&h->d_lch, sizeof(int) * L) == cudaSuccess && cudaMalloc(&h->d_lkind, sizeof(int) * L) == cudaSuccess &&
                cudaMalloc(&h->d_lshape, sizeof(double) * L * RICH_SP) == cudaSuccess &&
+               cudaMalloc(&h->d_wl_off, sizeof(int) * (L + 1)) == cudaSuccess && cudaMalloc(&h->d_wl_idx, sizeof(int) * R) == cudaSuccess &&
                cudaMalloc(&h->d_full, sizeof(double) * full_doubles) == cudaSuccess;
     if (!okr) {
       cudaGetLastError();
@@ -533,6 +541,8 @@ extern "C" pwa_status pwa_create_rich(const pwa_model_desc* m, const pwa_rich_de
         (ce = cudaMemcpyAsync(h->d_lch, rich->ls_chan, sizeof(int) * L, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
         (ce = cudaMemcpyAsync(h->d_lkind, kind.data(), sizeof(int) * L, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
         (ce = cudaMemcpyAsync(h->d_lshape, shape.data(), sizeof(double) * L * RICH_SP, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
+        (ce = cudaMemcpyAsync(h->d_wl_off, wl_off.data(), sizeof(int) * (L + 1), cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
+        (ce = cudaMemcpyAsync(h->d_wl_idx, wl_idx.data(), sizeof(int) * R, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
         (ce = cudaStreamSynchronize(h->stream)) != cudaSuccess)
       return fail_create(h, PWA_ERR_CUDA, std::string("upload: ") + cudaGetErrorString(ce));
   }
@@ -550,7 +560,8 @@ extern "C" pwa_status pwa_destroy(pwa_handle* h) {
   cudaStreamSynchronize(h->stream);
   for (void* p : h->owned) if (p) cudaFree(p);
   void* dev[] = {h->d_ch, h->d_K, h->d_partial, h->d_sums, h->d_raw, h->d_flags, h->d_io, h->d_fit, h->d_pcache, h->d_theta_keep, h->d_batch,
-                 h->d_map, h->d_csr_off, h->d_csr_idx, h->d_wres, h->d_lch, h->d_lkind, h->d_lshape, h->d_full};
+                 h->d_map, h->d_csr_off, h->d_csr_idx, h->d_wres, h->d_lch, h->d_lkind, h->d_lshape, h->d_full,
+                 h->d_wl_off, h->d_wl_idx};
   for (void* p : dev) if (p) cudaFree(p);
   for (cudaEvent_t e : h->prof_events) cudaEventDestroy(e);
   if (h->h_pin) cudaFreeHost(h->h_pin);

@@ -34,6 +34,8 @@ struct pwa_handle {
   int* d_lch = nullptr;         // [n_ls] channel of each resonance
   int* d_lkind = nullptr;       // [n_ls]
   double* d_lshape = nullptr;   // [n_ls][6]
+  int* d_wl_off = nullptr;      // [n_ls + 1] resonance -> range in d_wl_idx
+  int* d_wl_idx = nullptr;      // [n_res] waves of each resonance, ascending
   double* d_full = nullptr;     // theta_full [n_full] | v_full [n_full] | raw_full [4 + 4 n_full] | K [n_res][16]
 
   // scratch

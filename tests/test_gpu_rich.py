@@ -201,20 +201,16 @@ def test_fit_runs_on_the_general_lineshape_kernel(oracle_mod, env):
     gm.close()
 
 
-def test_per_wave_fractions_of_a_shared_resonance_model(oracle_mod, env):
-    """pwa_fit_fractions on a pwa_create_rich handle (constant widths): per-WAVE fractions at the expanded parameters,
-    against oracle/fractions.py on the base model the expansion defines."""
-    from oracle.fractions import fit_fractions
+@pytest.mark.parametrize("which", ["shared_const", "mixed"])
+def test_resonance_fractions_match_the_oracle(oracle_mod, env, which):
+    """pwa_fit_fractions on a pwa_create_rich handle: one coherent fraction per RESONANCE (Table 1 of the paper lists
+    one per resonance, PAPER.md:102-113), every lineshape kind, against oracle/fractions.py::fit_fractions_rich."""
+    from oracle.fractions import fit_fractions_rich
     pwa, rich = env
-    rm, gm = _shared_const(env, oracle_mod)
+    rm, gm = (_shared_const if which == "shared_const" else _mixed)(env, oracle_mod)
     th = _theta(4, rm.n_wave, rm.n_ls)
-    W = rm.n_wave
-    full = np.empty(4 * W)
-    full[0::4], full[1::4] = th[0:2 * W:2], th[1:2 * W:2]
-    full[2::4], full[3::4] = th[2 * W + 2 * rm.wave_res], th[2 * W + 2 * rm.wave_res + 1]
-    base = oracle_mod.Model(rm.res_chan[rm.wave_res], rm.data, rm.mc)
-    want = fit_fractions(base, full)
+    want = fit_fractions_rich(rm, th)
     got = gm.fit_fractions(th)
-    assert got.shape == (W,)
+    assert got.shape == (rm.n_ls,)
     assert np.max(np.abs(got - want)) <= 1e-10 * np.max(np.abs(want))
     gm.close()

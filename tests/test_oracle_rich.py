@@ -208,3 +208,36 @@ def test_r6_shared_resonance_is_the_base_model_expanded_and_contracted(oracle_mo
     assert abs(float(f1 - f0)) <= 1e-15 * abs(float(f0))
     assert rel_l2(g1, E.T @ np.asarray(g0, dtype=LD)) < 1e-14
     assert rel_l2(h1, E.T @ np.asarray(h0, dtype=LD)) < 1e-14
+
+
+# ----------------------------------------------------------------------------------------------- fractions
+def test_resonance_fractions_reduce_to_the_known_cases(oracle_mod, rich):
+    """fit_fractions_rich (one coherent fraction per resonance): one wave per constant-width resonance gives the base
+    per-resonance fractions (oracle/fractions.py, pinned by closed forms in test_oracle_fractions.py); two waves of ONE
+    resonance with identical projections give |c_1 + c_2|^2 B-weighted, i.e. the fraction of the merged wave; a model
+    with a single resonance has fraction 1 whatever its waves; global phase and common scale drop out."""
+    from oracle.fractions import fit_fractions, fit_fractions_rich
+    o = oracle_mod
+    W = 4
+    data, mc = _samples(o, 61, W, 2, 2, 10, 400)
+    res_chan = np.array([0, 1, 1, 0], dtype=np.int32)
+    rm = rich.RichModel(np.arange(W), res_chan, np.zeros(W), np.zeros((W, rich.N_SP)), data, mc)
+    th = _theta(5, W, W)
+    base_th = np.empty(4 * W)
+    base_th[0::4], base_th[1::4], base_th[2::4], base_th[3::4] = th[0:2 * W:2], th[1:2 * W:2], th[2 * W::2], th[2 * W + 1::2]
+    want = fit_fractions(o.Model(res_chan, data, mc), base_th)
+    assert np.max(np.abs(fit_fractions_rich(rm, th) - want)) <= 1e-14
+    # waves 0 and 1 identical, both in resonance 0 (Flatte), wave 2 in resonance 1
+    data, mc = _samples(o, 62, 3, 2, 1, 10, 300)
+    mc.amp[1] = mc.amp[0]
+    shape = np.zeros((2, rich.N_SP)); shape[0, :5] = (M_PI, M_PI, M_K, M_K, 4.21)
+    rm2 = rich.RichModel([0, 0, 1], [0, 0], [2, 0], shape, data, mc)
+    th2 = _theta(6, 3, 2)
+    c = th2[0] * np.exp(1j * th2[1]) + th2[2] * np.exp(1j * th2[3])
+    merged = th2.copy(); merged[0], merged[1], merged[2] = abs(c), np.angle(c), 0.0
+    f2, fm = fit_fractions_rich(rm2, th2), fit_fractions_rich(rm2, merged)
+    assert np.max(np.abs(f2 - fm)) <= 1e-13
+    gauge = th2.copy(); gauge[0:6:2] *= 2.5; gauge[1:6:2] -= 0.7
+    assert np.max(np.abs(fit_fractions_rich(rm2, gauge) - f2)) <= 1e-13
+    one = rich.RichModel([0, 0, 0], [0], [1], np.array([[M_PI, M_PI, 1.0, 0, 0, 0]]), data, mc)
+    assert abs(fit_fractions_rich(one, _theta(7, 3, 1))[0] - 1.0) <= 1e-14
