@@ -143,7 +143,7 @@ def _csrc_digest() -> str:
     import hashlib
     d = os.path.join(ROOT, "paper_2403_09225_b200", "csrc")
     hsh = hashlib.sha256()
-    for name in ("pwa_common.cuh", "pwa_kernels.cuh", "pwa_sweep_lanes.cuh", "pwa_sweep_lanes.cu"):
+    for name in ("pwa_common.cuh", "pwa_kernels.cuh", "pwa_sweep_lanes.cuh", "pwa_sweep_lanes.cu", "pwa_sweep_pair.cuh"):
         with open(os.path.join(d, name), "rb") as f:
             hsh.update(name.encode() + b"\0" + f.read())
     return hsh.hexdigest()[:16]

@@ -83,8 +83,9 @@ static pwa_status raw_sums_impl(pwa_handle* h, int mode, const double* theta, co
   int nb = 0;
   if (packed) {
     // lanes sweep: the per-resonance constants are formed by every block itself (no prologue launch)
+    if (mode == MODE_FULL && pair_available(h)) mode = MODE_FULLP;  // two events per lane (pwa_sweep_pair.cuh)
     if (prof) cudaEventRecord(h->prof_events[h->prof_used], h->stream);
-    pwa_status st = lanes_launch(h, mode, theta, mode_q(mode) ? v : nullptr, skip);
+    pwa_status st = mode == MODE_FULLP ? pair_launch(h, theta, v, skip) : lanes_launch(h, mode, theta, mode_q(mode) ? v : nullptr, skip);
     if (st != PWA_OK) return st;
     h->launches++;
     if (prof) {
@@ -124,6 +125,7 @@ static pwa_status raw_sums_impl(pwa_handle* h, int mode, const double* theta, co
     case MODE_GRAD: PWA_REDUCE(MODE_GRAD); break;
     case MODE_GRAD3: PWA_REDUCE(MODE_GRAD3); break;
     case MODE_HVPQ: PWA_REDUCE(MODE_HVPQ); break;
+    case MODE_FULLP: PWA_REDUCE(MODE_FULLP); break;
     default: PWA_REDUCE(MODE_FULL); break;
   }
 #undef PWA_REDUCE

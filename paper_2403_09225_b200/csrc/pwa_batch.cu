@@ -1,14 +1,74 @@
 // pwa_batch.cu - host side of the batch sweeps (pwa_batch.cuh): kernel lookup, shared-memory plan, launch.
 #include <algorithm>
+#include <cstdlib>
 
 #include "pwa_internal.h"
 #include "pwa_batch.cuh"
+#include "pwa_sweep_pair.cuh"
 
 namespace pwa {
 
 namespace {
 inline unsigned up(unsigned x, unsigned m) { return (x + m - 1) / m * m; }
 }  // namespace
+
+// ---- the fused sweep with two events per lane (pwa_sweep_pair.cuh) -------------------------------------------------
+static pair_fn pair_kernel(const pwa_handle* h) {
+  if (h->variant < 2 || h->lanes_combo < 0) return nullptr;
+  const LanesCombo& c = kLanesCombos[h->lanes_combo];
+  if (!(c.rho == 4 && c.log_sw == 3 && c.nw == 8 && c.prod == 2 && c.tile == 32)) return nullptr;
+  static const bool off = std::getenv("PWA_PAIR") && std::atoi(std::getenv("PWA_PAIR")) == 0;  // A/B runs
+  if (off) return nullptr;
+  switch (h->n_hel) {
+    case 1: return pair_kernel_h1();
+    case 2: return pair_kernel_h2();
+  }
+  return nullptr;
+}
+
+static bool pair_plan(const pwa_handle* h, PairArgs& p, size_t& smem) {
+  const int NW = 8, EW = 4, RP = 32, H = h->n_hel;
+  int dev_smem = 0;
+  cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device);
+  const unsigned k_bytes = up((unsigned)RP * lanes::KSP * 8, 128);
+  const unsigned red_bytes = up((unsigned)NW * (h->n_res * 8 + 2) * 8, 128);
+  const unsigned xch_bytes = up((unsigned)NW * 2 * EW * (4 * H + 2) * 8, 128);
+  const unsigned fixed = k_bytes + red_bytes + xch_bytes + 32u * 2 * 8 + 128;
+  const long long fit = ((long long)dev_smem - fixed) / h->largs.stage_bytes;
+  const int stages = (int)std::min<long long>(fit, h->largs.stages);
+  if (stages < 3) return false;
+  p.stages = stages;
+  p.off_K = (unsigned)stages * h->largs.stage_bytes;
+  p.off_red = p.off_K + k_bytes;
+  p.off_xch = p.off_red + red_bytes;
+  p.off_bar = p.off_xch + xch_bytes;
+  smem = (size_t)stages * h->largs.stage_bytes + fixed;
+  return true;
+}
+
+bool pair_available(const pwa_handle* h) {
+  if (!pair_kernel(h)) return false;
+  PairArgs p;
+  size_t smem;
+  return pair_plan(h, p, smem);
+}
+
+pwa_status pair_launch(pwa_handle* h, const double* theta, const double* v, const double* skip) {
+  pair_fn fn = pair_kernel(h);
+  PairArgs p;
+  size_t smem = 0;
+  if (!fn || !pair_plan(h, p, smem)) return set_error(h, PWA_ERR_INVALID_ARG, "no two-event kernel for this shape", cudaSuccess);
+  cudaError_t ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (ce != cudaSuccess) return set_error(h, PWA_ERR_CUDA, "cudaFuncSetAttribute(two-event sweep)", ce);
+  LaneArgs a = h->largs;
+  a.theta = theta;
+  a.v = v;
+  a.skip = skip;
+  a.partial = h->d_partial;
+  fn<<<h->grid, lanes::lanes_threads(8, 2), smem, h->stream>>>(a, p);
+  if ((ce = cudaGetLastError()) != cudaSuccess) return set_error(h, PWA_ERR_CUDA, "launch two-event sweep kernel", ce);
+  return PWA_OK;
+}
 
 // ---- batch sweeps (pwa_batch.cuh) ---------------------------------------------------------------------------
 static batch_fn batch_kernel(const pwa_handle* h, int kind, int kb) {

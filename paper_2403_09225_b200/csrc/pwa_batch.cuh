@@ -182,13 +182,13 @@ __global__ void __launch_bounds__(lanes_threads(NW, 2), 1) k_batch_lanes(const _
     double* xrowp = reinterpret_cast<double*>(smem_raw + b.off_xch) + ((size_t)w * EW + e) * (NV + 2) +
                     (size_t)(s & 1) * ((size_t)NW * EW * (NV + 2));  // second half of the buffer: odd slices' events
     int t = w / NPP;
+    int st = t % stages, ph = (t / stages) & 1;
     for (int smp = 0; smp < 2; ++smp) {
       const int t_end = smp ? T : TmB;
       const int n = (int)(smp ? nD : nM);
       const bool weighted = smp == 1 && a.weighted;
 #pragma unroll 1
       while (t < t_end) {
-        const int st = t % stages, ph = (t / stages) & 1;
         const int i0 = (bk + (t - (smp ? TmB : 0)) * G) * TILE;
         const bool valid = i0 + evA < n;
         mbar_wait(full0 + 8 * st, (uint32_t)ph);
@@ -265,6 +265,11 @@ __global__ void __launch_bounds__(lanes_threads(NW, 2), 1) k_batch_lanes(const _
         }
         if (smp == 1) s1 += wv;
         t += NW / NPP;
+        st += NW / NPP;
+        if (st >= stages) {
+          st -= stages;
+          ph ^= 1;
+        }
       }
       // end of a sample: the lanes of slices 0 and 1 (lane < 2 EW) hold every event of the warp's columns once
       double* out = b.partial + ((size_t)smp * gridDim.x + blockIdx.x) * (size_t)row_len;

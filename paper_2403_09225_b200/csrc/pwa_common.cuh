@@ -24,13 +24,14 @@ enum { K_M2 = 0, K_Y2 = 1, K_Y = 2, K_CR = 4, K_CI = 5, K_AR = 6, K_AI = 7, K_BR
 // MODE_GRAD3 and MODE_HVPQ split the fused sweep for Newton-CG: at a fixed theta the compact sums
 // P1, P2, P3 do not depend on the direction v, so the gradient evaluation of an outer iteration keeps them (GRAD3) and
 // every CG iteration only accumulates Q1, Q2 (HVPQ): 49 instead of 69 FP64 instructions per (event, resonance).
-enum Mode { MODE_NLL = 0, MODE_GRAD = 1, MODE_FULL = 2, MODE_GRAD3 = 3, MODE_HVPQ = 4 };
-__host__ __device__ constexpr bool mode_p(int m) { return m == MODE_GRAD || m == MODE_FULL || m == MODE_GRAD3; }   // P1, P2
+// MODE_FULLP: the fused sweep with P3 folded into Q2 (pwa_sweep_pair.cuh): P1, P2, Q1, Q2' = Q2 + 2 lambda P3 per resonance
+enum Mode { MODE_NLL = 0, MODE_GRAD = 1, MODE_FULL = 2, MODE_GRAD3 = 3, MODE_HVPQ = 4, MODE_FULLP = 5 };
+__host__ __device__ constexpr bool mode_p(int m) { return m == MODE_GRAD || m == MODE_FULL || m == MODE_GRAD3 || m == MODE_FULLP; }   // P1, P2
 __host__ __device__ constexpr bool mode_p3(int m) { return m == MODE_FULL || m == MODE_GRAD3; }                     // P3
-__host__ __device__ constexpr bool mode_q(int m) { return m == MODE_FULL || m == MODE_HVPQ; }  // Adot, Q1, Q2 (needs v)
+__host__ __device__ constexpr bool mode_q(int m) { return m == MODE_FULL || m == MODE_HVPQ || m == MODE_FULLP; }  // Adot, Q1, Q2 (needs v)
 
 // values per resonance that the backward pass produces, and resonances per 32-value batch
-__host__ __device__ constexpr int vpr_of(int mode) { return mode == MODE_FULL ? 10 : (mode == MODE_GRAD3 ? 6 : 4); }
+__host__ __device__ constexpr int vpr_of(int mode) { return mode == MODE_FULL ? 10 : (mode == MODE_FULLP ? 8 : (mode == MODE_GRAD3 ? 6 : 4)); }
 __host__ __device__ constexpr int rpb_of(int mode) { return mode == MODE_FULL ? 3 : 8; }
 
 struct SampleDev {

@@ -434,6 +434,10 @@ __global__ void __launch_bounds__(1024) k_reduce_unpack(const double* __restrict
             s.Q1 = {__ldcg(q + 6), __ldcg(q + 7)};
             s.Q2 = {__ldcg(q + 8), __ldcg(q + 9)};
           }
+          if (MODE == MODE_FULLP) {  // Q2 holds Q2 + 2 lambda P3: with P3 = 0 the unpacking below is unchanged
+            s.Q1 = {__ldcg(q + 4), __ldcg(q + 5)};
+            s.Q2 = {__ldcg(q + 6), __ldcg(q + 7)};
+          }
         }
         double g4[4], h4[4] = {0.0, 0.0, 0.0, 0.0};
         unpack_res(s, a, phi, M, G, (mode_q(MODE) && v) ? v + 4 * r : nullptr, g4, h4);

@@ -2,6 +2,7 @@
 // the four counts compile in parallel (build.py).  The (RHO, LOG_SW, NW) table must match kLanesCombos in pwa_internal.h.
 #include "pwa_internal.h"
 #include "pwa_batch.cuh"
+#include "pwa_sweep_pair.cuh"
 
 #ifndef PWA_LANES_H
 #error "compile with -DPWA_LANES_H=<n_hel>"
@@ -41,6 +42,15 @@ lanes_fn PWA_CAT(lanes_kernel_h, PWA_LANES_H)(int combo, int mode) {
     case 13: return for_mode<5, 1, 8, 2>(mode);
   }
   return nullptr;
+}
+
+// two events per lane (pwa_sweep_pair.cuh): the fused sweep of the (4 x 8 slices) shape, H <= 2 (two events' G fit the registers)
+pair_fn PWA_CAT(pair_kernel_h, PWA_LANES_H)() {
+#if PWA_LANES_H <= 2
+  return lanes::k_sweep_pair<PWA_LANES_H>;
+#else
+  return nullptr;
+#endif
 }
 
 // batch kernels (pwa_batch.cuh): only the warpgroup shapes (8 compute warps, 32-event tiles); kb: sets / directions per pass
