@@ -164,7 +164,7 @@ def _stored_traffic(config: int, variant: str):
                     if len(parts) >= 3 and parts[0] == f"config{config}" and parts[1] == variant:
                         if len(parts) >= 4 and parts[3] == digest:
                             return float(parts[2]), f"profiles/{name} (ncu --set full, csrc digest {digest})"
-                        stale = f"profiles/{name} was captured on other kernel sources (csrc digest now {digest})"
+                        stale = stale or f"profiles/{name} was captured on other kernel sources (csrc digest now {digest})"
         except (OSError, ValueError):
             continue
     return None, stale or f"no ncu capture for config{config};{variant};{digest} under profiles/"
