@@ -17,8 +17,8 @@ static pair_fn pair_kernel(const pwa_handle* h) {
   if (h->variant < 2 || h->lanes_combo < 0) return nullptr;
   const LanesCombo& c = kLanesCombos[h->lanes_combo];
   if (!(c.rho == 4 && c.log_sw == 3 && c.nw == 8 && c.prod == 2 && c.tile == 32)) return nullptr;
-  static const bool off = std::getenv("PWA_PAIR") && std::atoi(std::getenv("PWA_PAIR")) == 0;  // A/B runs
-  if (off) return nullptr;
+  const char* env = std::getenv("PWA_PAIR");  // PWA_PAIR=0: the one-event kernel (A/B runs, tests of that path)
+  if (env && std::atoi(env) == 0) return nullptr;
   switch (h->n_hel) {
     case 1: return pair_kernel_h1();
     case 2: return pair_kernel_h2();

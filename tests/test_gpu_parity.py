@@ -219,6 +219,25 @@ def test_every_kernel_shape_matches_oracle(pwa, oracle_mod, case, combo, monkeyp
         gm.close()
 
 
+def test_one_event_fused_kernel_of_the_config3_shape(pwa, oracle_mod, monkeypatch):
+    """The fused calls of the 4 x 8-slice shape run the two-events-per-lane kernel (csrc/pwa_sweep_pair.cuh); PWA_PAIR=0
+    keeps the one-event kernel of the same shape reachable - both against the oracle, and against each other (the two
+    sum in a different order: equal to rounding, not bit for bit)."""
+    import workloads
+    cfg, w, om, gm = _case(pwa, oracle_mod, *CASES[2])
+    th, v = _thetas(cfg)[3], workloads.direction(cfg, 11).numpy()
+    f0, g0, h0 = oracle_mod.nll_grad_hvp(om, th, v, "ld")
+    l0 = pwa.pwa_kernel_launches(gm.h)
+    f2, g2, h2 = gm.nll_grad_hvp(th, v)
+    assert pwa.pwa_kernel_launches(gm.h) - l0 == 2
+    monkeypatch.setenv("PWA_PAIR", "0")
+    f1, g1, h1 = gm.nll_grad_hvp(th, v)
+    monkeypatch.delenv("PWA_PAIR")
+    for f, g, hv in ((f1, g1, h1), (f2, g2, h2)):
+        assert _nll_err(f, f0) < NLL_TOL and rel_l2(g, g0) < VEC_TOL and rel_l2(hv, h0) < VEC_TOL
+    assert rel_l2(g1, g2) < 1e-12 and rel_l2(h1, h2) < 1e-12 and (g1.tobytes() != g2.tobytes() or h1.tobytes() != h2.tobytes())
+
+
 def test_many_repeats_bit_identical_under_load(pwa, oracle_mod):
     """A race in the TMA ring, the shared-memory exchange rows or the ticketed reduction would show up as a changed
     bit in some repeat (compute-sanitizer is not available on the GPU pool).  150 back-to-back evaluations in all
