@@ -75,7 +75,7 @@ static size_t generic_smem(int block, int nb) { return (size_t)(block / 32) * ((
 // Runs prologue + sweep + stage-2 reduction/unpack; leaves the public raw vector in `raw` (device).
 static pwa_status raw_sums_impl(pwa_handle* h, int mode, const double* theta, const double* v, double* raw,
                                 bool combine = false, double* nll = nullptr, double* grad = nullptr, double* hv = nullptr,
-                                const double* skip = nullptr) {
+                                const double* skip = nullptr, const CgTail* cg = nullptr) {
   const int R = h->n_res;
   if (mode == MODE_FULL && !v) mode = MODE_GRAD;
   const bool prof = h->profiling && h->prof_used + 2 <= h->prof_events.size();
@@ -116,10 +116,12 @@ static pwa_status raw_sums_impl(pwa_handle* h, int mode, const double* theta, co
     if (cudaError_t ce = cudaGetLastError()) return set_error(h, PWA_ERR_CUDA, "launch sweep kernel", ce);
   }
   const double n_mc = (double)h->smp[0].n;
+  CgTail cgt = {};
+  if (cg && mode == MODE_HVPQ && combine) cgt = *cg;
 #define PWA_REDUCE(M)                                                                                              \
   k_reduce_unpack<M><<<kReduceBlocks, 1024, 0, h->stream>>>(h->d_partial, h->grid, nb, R, packed, theta, v, n_mc,  \
                                                              h->d_sums, raw, combine ? 1 : 0, nll, grad, hv,        \
-                                                             h->d_flags, h->d_flags + 1, h->d_pcache, skip)
+                                                             h->d_flags, h->d_flags + 1, h->d_pcache, skip, cgt)
   switch (mode) {
     case MODE_NLL: PWA_REDUCE(MODE_NLL); break;
     case MODE_GRAD: PWA_REDUCE(MODE_GRAD); break;
@@ -276,14 +278,14 @@ pwa_status eval_grad_keep(pwa_handle* h, const double* theta, double* nll, doubl
   return st;
 }
 
-pwa_status eval_hvp_kept(pwa_handle* h, const double* v, double* hv, const double* skip) {
+pwa_status eval_hvp_kept(pwa_handle* h, const double* v, double* hv, const double* skip, const CgTail* cg) {
   if (!h->keep_valid) return set_error(h, PWA_ERR_INVALID_ARG, "pwa_hvp_cached: no pwa_nll_grad_for_hvp call before", cudaSuccess);
   if (h->mapped) {
     const int mode = (h->rich_kernel || h->variant < 2) ? MODE_FULL : MODE_HVPQ;
     return eval_mapped(h, mode, nullptr, v, h->d_raw, true, nullptr, nullptr, hv);
   }
   if (h->variant < 2) return eval(h, MODE_FULL, h->d_theta_keep, v, nullptr, nullptr, hv);
-  return raw_sums_impl(h, MODE_HVPQ, h->d_theta_keep, v, h->d_raw, true, nullptr, nullptr, hv, skip);
+  return raw_sums_impl(h, MODE_HVPQ, h->d_theta_keep, v, h->d_raw, true, nullptr, nullptr, hv, skip, cg);
 }
 
 }  // namespace pwa

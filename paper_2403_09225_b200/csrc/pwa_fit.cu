@@ -9,6 +9,7 @@
 #include <math_constants.h>
 
 #include "pwa_internal.h"
+#include "pwa_kernels.cuh"
 
 namespace {
 
@@ -264,24 +265,27 @@ extern "C" pwa_status pwa_fit_newton_cg(pwa_handle* h, double* theta, const pwa_
     int done_at = -1;
     double cg_end = 0.0;
     for (int j = 0; j < o.max_cg; ++j) {
-      FIT_EVAL(pwa::eval_hvp_kept(h, d, q, pipelined ? sc + S_STATUS : nullptr));
-      k_cg_iter<<<1, FT, 0, st>>>(P, j, g, mask, q, z, r, d, p, sc);
-      h->launches++;
-      if (!pipelined) {
-        FIT_CHECK(fetch());
-        if (hs[S_STATUS] != 0.0) { done_at = j; cg_end = hs[S_STATUS]; break; }
+      if (pipelined) {
+        // the CG update runs in the tail of the HVP's reduction launch and leaves its verdict in mapped pinned memory:
+        // per iteration two launches (sweep, reduction + CG) and an event, no copy
+        const pwa::CgTail cg = {g, mask, z, r, d, p, sc, hs + S_N + (j & 1), P, j};
+        FIT_EVAL(pwa::eval_hvp_kept(h, d, q, sc + S_STATUS, &cg));
+        FIT_CHECK(cudaEventRecord(ev[j & 1], st));
+        if (j >= 1) {
+          FIT_CHECK(cudaEventSynchronize(ev[(j - 1) & 1]));
+          if (hs[S_N + ((j - 1) & 1)] != 0.0) { done_at = j - 1; cg_end = hs[S_N + ((j - 1) & 1)]; break; }
+        }
+        if (j == o.max_cg - 1) {
+          FIT_CHECK(cudaEventSynchronize(ev[j & 1]));
+          if (hs[S_N + (j & 1)] != 0.0) { done_at = j; cg_end = hs[S_N + (j & 1)]; }
+        }
         continue;
       }
-      FIT_CHECK(cudaMemcpyAsync(hs + S_N + (j & 1), sc + S_STATUS, sizeof(double), cudaMemcpyDeviceToHost, st));
-      FIT_CHECK(cudaEventRecord(ev[j & 1], st));
-      if (j >= 1) {
-        FIT_CHECK(cudaEventSynchronize(ev[(j - 1) & 1]));
-        if (hs[S_N + ((j - 1) & 1)] != 0.0) { done_at = j - 1; cg_end = hs[S_N + ((j - 1) & 1)]; break; }
-      }
-      if (j == o.max_cg - 1) {
-        FIT_CHECK(cudaEventSynchronize(ev[j & 1]));
-        if (hs[S_N + (j & 1)] != 0.0) { done_at = j; cg_end = hs[S_N + (j & 1)]; }
-      }
+      FIT_EVAL(pwa::eval_hvp_kept(h, d, q, nullptr));
+      k_cg_iter<<<1, FT, 0, st>>>(P, j, g, mask, q, z, r, d, p, sc);
+      h->launches++;
+      FIT_CHECK(fetch());
+      if (hs[S_STATUS] != 0.0) { done_at = j; cg_end = hs[S_STATUS]; break; }
     }
     have_p = done_at >= 0;
     const int iters = have_p ? done_at + 1 : o.max_cg;

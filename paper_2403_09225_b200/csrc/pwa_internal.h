@@ -127,7 +127,9 @@ pwa_status lanes_launch(pwa_handle* h, int mode, const double* theta, const doub
 pwa_status eval(pwa_handle* h, int mode, const double* theta, const double* v, double* nll, double* grad,
                 double* hv);
 pwa_status eval_grad_keep(pwa_handle* h, const double* theta, double* nll, double* grad);
-pwa_status eval_hvp_kept(pwa_handle* h, const double* v, double* hv, const double* skip = nullptr);  // skip: LaneArgs::skip
+struct CgTail;  // pwa_kernels.cuh: a CG iteration run in the tail of the HVP's reduction launch (lanes variant, plain handles)
+pwa_status eval_hvp_kept(pwa_handle* h, const double* v, double* hv, const double* skip = nullptr,  // skip: LaneArgs::skip
+                         const CgTail* cg = nullptr);
 pwa_status set_error(pwa_handle* h, pwa_status st, const char* what, cudaError_t ce);
 pwa_status expand_theta(pwa_handle* h, const double* theta);  // rich handles: h->d_full[0 .. n_full) <- theta expanded
 }  // namespace pwa

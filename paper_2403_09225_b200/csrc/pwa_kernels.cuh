@@ -348,6 +348,74 @@ static __global__ void __launch_bounds__(1024) k_combine(const double* raw, cons
   combine_block(raw, v, P, nll, grad, hv, flags);
 }
 
+// One truncated-CG iteration of the fit driver (pwa_fit.cu, step 3 of DESIGN.md S15'), run by the block that has just
+// written q = H d (the tail of k_reduce_unpack<MODE_HVPQ>): one launch, one launch gap and one status copy less per CG
+// iteration than a kernel of its own.  sc: the driver's scalar block (rr at [2], eps at [5], status at [6]); status
+// 0 continue, 1 non-positive curvature, 2 residual small; on status != 0 the step p is written.  host_status: mapped
+// pinned memory the host reads after its event (nullptr: none).  g == nullptr: no CG work in this launch.
+struct CgTail {
+  const double* g;
+  const double* mask;
+  double *z, *r, *d, *p, *sc;
+  double* host_status;
+  int P, j;
+};
+
+__device__ __forceinline__ double block_sum_1024(double x, double* red) {
+  red[threadIdx.x] = x;
+  __syncthreads();
+  for (int s = blockDim.x / 2; s > 0; s >>= 1) {
+    if ((int)threadIdx.x < s) red[threadIdx.x] += red[threadIdx.x + s];
+    __syncthreads();
+  }
+  const double r = red[0];
+  __syncthreads();
+  return r;
+}
+
+__device__ inline void cg_iter_block(const CgTail& c, const double* q) {
+  __shared__ double red[1024];
+  const int P = c.P, nt = blockDim.x;
+  double dq = 0.0, dd = 0.0;
+  for (int k = threadIdx.x; k < P; k += nt) {
+    dq = fma(c.d[k], q[k] * c.mask[k], dq);
+    dd = fma(c.d[k], c.d[k], dd);
+  }
+  dq = block_sum_1024(dq, red);
+  dd = block_sum_1024(dd, red);
+  const double rr = c.sc[2], eps = c.sc[5];
+  double status = 0.0;
+  if (!(dq > 1e-14 * dd)) {  // also catches NaN
+    for (int k = threadIdx.x; k < P; k += nt) c.p[k] = (c.j == 0) ? -c.g[k] * c.mask[k] : c.z[k];
+    status = 1.0;
+  } else {
+    const double alpha = rr / dq;
+    double rn = 0.0;
+    for (int k = threadIdx.x; k < P; k += nt) {
+      c.z[k] = fma(alpha, c.d[k], c.z[k]);
+      const double rk = fma(alpha, q[k] * c.mask[k], c.r[k]);
+      c.r[k] = rk;
+      rn = fma(rk, rk, rn);
+    }
+    rn = block_sum_1024(rn, red);
+    if (sqrt(rn) <= eps) {
+      for (int k = threadIdx.x; k < P; k += nt) c.p[k] = c.z[k];
+      status = 2.0;
+    } else {
+      const double beta = rn / rr;
+      for (int k = threadIdx.x; k < P; k += nt) c.d[k] = fma(beta, c.d[k], -c.r[k]);
+      if (threadIdx.x == 0) c.sc[2] = rn;
+    }
+  }
+  if (threadIdx.x == 0) {
+    c.sc[6] = status;
+    if (c.host_status) {
+      *c.host_status = status;
+      __threadfence_system();
+    }
+  }
+}
+
 // Second reduction stage (a-7): fixed-order sum of the per-block partial rows, compact sums -> raw sums
 // (SURVEY appendix), and - when `combine` is set - Eqs. 4, 6, 7 in the same launch (the evaluation calls; the
 // shard interface pwa_raw_sums stops at the raw vector).
@@ -358,7 +426,8 @@ __global__ void __launch_bounds__(1024) k_reduce_unpack(const double* __restrict
                                                         const double* __restrict__ v, double n_mc, double* sums, double* raw,
                                                         int combine, double* __restrict__ nll, double* __restrict__ grad,
                                                         double* __restrict__ hv, unsigned* __restrict__ flags,
-                                                        unsigned* ticket, double* pcache, const double* skip) {
+                                                        unsigned* ticket, double* pcache, const double* skip,
+                                                        const CgTail cg) {
   if (skip != nullptr && *skip != 0.0) return;  // see LaneArgs::skip
   constexpr int VPR = vpr_of(MODE), RPB = rpb_of(MODE);
   const int nacc = packed ? (MODE == MODE_NLL ? 0 : R * VPR) : nb * 32, stride = nacc + 2, P = 4 * R;
@@ -454,6 +523,10 @@ __global__ void __launch_bounds__(1024) k_reduce_unpack(const double* __restrict
   if (combine) {
     __syncthreads();  // the raw vector of this block's own writes is visible to the whole block
     combine_block(raw, mode_q(MODE) ? v : nullptr, P, nll, grad, mode_q(MODE) ? hv : nullptr, flags);
+    if (MODE == MODE_HVPQ && cg.g != nullptr) {
+      __syncthreads();  // hv = q = H d of this block's own writes
+      cg_iter_block(cg, hv);
+    }
   }
 }
 
