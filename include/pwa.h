@@ -9,15 +9,20 @@
  *   NLL(theta) = - sum_data w_i ln I_i + W ln( sum_mc I_j / N_mc ),  W = sum_data w_i
  *                                                                            PAPER.md:67 (Eq. 3), S2, S3
  *   grad NLL, and (Hessian of NLL) . v for a given direction v               PAPER.md:90 (Eq. 6), :95 (Eq. 7, S9)
- *   a truncated line-search Newton-CG minimisation of NLL                    PAPER.md:27, :119; DESIGN.md (c-F)
+ *   a projected, truncated line-search Newton-CG minimisation of NLL         PAPER.md:27, :43, :119; S15', S19
+ *   K values / K Hessian-vector products in one pass over the events, the Hessian matrix (pwa_nll_batch ...)
+ *   additive raw sums of an event shard and their combination (Eqs. 4-7), fit fractions (S20)
+ *   optionally (pwa_create_rich): partial waves sharing a resonance's lineshape, mass-dependent width, Flatte (S21, S22)
  *
- * Parameters: theta[4r..4r+3] = (a_r, phi_r, M_r, Gamma_r), r = 0..n_res-1 (S6); P = 4*n_res doubles.
+ * Parameters: theta[4r..4r+3] = (a_r, phi_r, M_r, Gamma_r), r = 0..n_res-1 (S6); P = 4*n_res doubles
+ * (pwa_create_rich handles: [a, phi per wave | M, Gamma per resonance], P = 2 n_res + 2 n_lineshape).
  * F_rh(i) ("amp") is the parameter-free projection of PAPER.md:70, an input computed once by the caller.
  *
  * Conventions
- *   - Every call returns a pwa_status; nothing throws across this boundary; no global state except a
- *     process-wide count of live handles.  One handle = one device + one stream; a handle is not
- *     thread-safe, different handles are independent.
+ *   - Every call returns a pwa_status; nothing throws across this boundary; no global state.  One handle = one device
+ *     + one stream; a handle is not thread-safe, different handles are independent.  Every call binds the calling
+ *     thread to the handle's device for its duration and restores the caller's current device before it returns, so
+ *     a handle may be used from any host thread (one thread per GPU).
  *   - There is no CPU path.  If no CUDA device is usable, pwa_create fails with PWA_ERR_CUDA.
  *   - Evaluation calls (pwa_nll ... pwa_raw_sums, pwa_combine) only ENQUEUE work on the handle's stream
  *     and return; they never synchronise.  Their theta / v / output pointers are DEVICE pointers that
