@@ -300,6 +300,15 @@ def run_fits(args):
                                    f"{K} fit(s) in flight",
                        "kernel_variant": pwa.pwa_kernel_variant(m.h)},
             "fits_converged": sum(1 for r in rows if r["status"] == 0),
+            # roofline-style account of a fit: every sweep (value, gradient or HVP) reads the event store once
+            "roofline_fit": (lambda nb, pk: {"bound": "hbm", "unit": "GB/s", "peak": pk[0], "peak_source": pk[1],
+                                             "bytes_per_sweep": nb,
+                                             "achieved": sum(r["sweeps"] for r in rows) * nb / t_all / 1e9,
+                                             "frac": sum(r["sweeps"] for r in rows) * nb / t_all / 1e9 / pk[0],
+                                             "us_per_sweep": 1e6 * t_all / max(1, sum(r["sweeps"] for r in rows)),
+                                             "what": "algorithmic bytes of all sweeps of all fits / wall time of the fits "
+                                                     "(host loop, reductions and CG updates included)"})(
+                pwa.pwa_bytes_per_eval(m.h), _peaks()),
             "sweeps_total": sum(r["sweeps"] for r in rows), "gpu_launches": int(launches),
             "fit_from_theta_true": {"nll": r_true.nll, "outer": r_true.outer_iters, "hvp": r_true.n_hvp,
                                     "seconds": r_true.seconds, "status": r_true.status},
