@@ -14,7 +14,9 @@ SHAPES = [(1, 1, 1, 1, 1, False), (1, 1, 1, 33, 65, True), (2, 4, 1, 7, 100, Tru
           (5, 2, 2, 257, 1000, True), (12, 1, 3, 100, 999, False), (13, 2, 3, 100, 999, True), (16, 4, 2, 64, 640, False),
           (17, 3, 1, 65, 700, True), (32, 2, 3, 129, 1025, True), (33, 2, 2, 90, 800, False), (33, 4, 3, 90, 515, True),
           (64, 1, 3, 50, 600, False), (65, 3, 2, 40, 400, True), (128, 4, 3, 33, 300, False), (129, 2, 3, 33, 300, True),
-          (6, 5, 2, 50, 500, True), (3, 8, 1, 20, 333, False)]
+          (6, 5, 2, 50, 500, True), (3, 8, 1, 20, 333, False),
+          # the two-events-per-lane fused kernel (13 <= R <= 32, H <= 2): H = 1, one event, fewer tiles than blocks and warps
+          (20, 1, 2, 70, 900, True), (30, 2, 3, 1, 1, False), (25, 2, 1, 33, 65, True), (32, 1, 3, 31, 4777, False)]
 
 
 @pytest.fixture(scope="module")
