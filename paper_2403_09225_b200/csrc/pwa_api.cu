@@ -83,9 +83,11 @@ static pwa_status raw_sums_impl(pwa_handle* h, int mode, const double* theta, co
   int nb = 0;
   if (packed) {
     // lanes sweep: the per-resonance constants are formed by every block itself (no prologue launch)
-    if (mode == MODE_FULL && pair_available(h)) mode = MODE_FULLP;  // two events per lane (pwa_sweep_pair.cuh)
+    if (mode == MODE_FULL && pair_available(h, MODE_FULLP)) mode = MODE_FULLP;  // two events per lane (pwa_sweep_pair.cuh)
+    const bool pair = pair_available(h, mode);  // every mode of the 4 x 8-slice shape with H <= 2
     if (prof) cudaEventRecord(h->prof_events[h->prof_used], h->stream);
-    pwa_status st = mode == MODE_FULLP ? pair_launch(h, theta, v, skip) : lanes_launch(h, mode, theta, mode_q(mode) ? v : nullptr, skip);
+    pwa_status st = pair ? pair_launch(h, mode, theta, mode_q(mode) ? v : nullptr, skip)
+                         : lanes_launch(h, mode, theta, mode_q(mode) ? v : nullptr, skip);
     if (st != PWA_OK) return st;
     h->launches++;
     if (prof) {

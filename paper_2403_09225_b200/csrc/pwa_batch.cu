@@ -13,15 +13,15 @@ inline unsigned up(unsigned x, unsigned m) { return (x + m - 1) / m * m; }
 }  // namespace
 
 // ---- the fused sweep with two events per lane (pwa_sweep_pair.cuh) -------------------------------------------------
-static pair_fn pair_kernel(const pwa_handle* h) {
+static pair_fn pair_kernel(const pwa_handle* h, int mode) {
   if (h->variant < 2 || h->lanes_combo < 0) return nullptr;
   const LanesCombo& c = kLanesCombos[h->lanes_combo];
   if (!(c.rho == 4 && c.log_sw == 3 && c.nw == 8 && c.prod == 2 && c.tile == 32)) return nullptr;
   const char* env = std::getenv("PWA_PAIR");  // PWA_PAIR=0: the one-event kernel (A/B runs, tests of that path)
   if (env && std::atoi(env) == 0) return nullptr;
   switch (h->n_hel) {
-    case 1: return pair_kernel_h1();
-    case 2: return pair_kernel_h2();
+    case 1: return pair_kernel_h1(mode);
+    case 2: return pair_kernel_h2(mode);
   }
   return nullptr;
 }
@@ -46,15 +46,15 @@ static bool pair_plan(const pwa_handle* h, PairArgs& p, size_t& smem) {
   return true;
 }
 
-bool pair_available(const pwa_handle* h) {
-  if (!pair_kernel(h)) return false;
+bool pair_available(const pwa_handle* h, int mode) {
+  if (!pair_kernel(h, mode)) return false;
   PairArgs p;
   size_t smem;
   return pair_plan(h, p, smem);
 }
 
-pwa_status pair_launch(pwa_handle* h, const double* theta, const double* v, const double* skip) {
-  pair_fn fn = pair_kernel(h);
+pwa_status pair_launch(pwa_handle* h, int mode, const double* theta, const double* v, const double* skip) {
+  pair_fn fn = pair_kernel(h, mode);
   PairArgs p;
   size_t smem = 0;
   if (!fn || !pair_plan(h, p, smem)) return set_error(h, PWA_ERR_INVALID_ARG, "no two-event kernel for this shape", cudaSuccess);

@@ -105,12 +105,13 @@ lanes_fn lanes_kernel(int H, int combo, int mode);
 // the fused sweep with two events per lane (pwa_sweep_pair.cuh); nullptr where it is not instantiated
 struct PairArgs;
 typedef void (*pair_fn)(const LaneArgs, const PairArgs);
-pair_fn pair_kernel_h1();
-pair_fn pair_kernel_h2();
-pair_fn pair_kernel_h3();
-pair_fn pair_kernel_h4();
-bool pair_available(const pwa_handle* h);  // the handle's shape has a two-event kernel (PWA_PAIR=0 switches it off)
-pwa_status pair_launch(pwa_handle* h, const double* theta, const double* v, const double* skip);
+pair_fn pair_kernel_h1(int mode);
+pair_fn pair_kernel_h2(int mode);
+pair_fn pair_kernel_h3(int mode);
+pair_fn pair_kernel_h4(int mode);
+// the handle's shape has a two-event kernel for this mode (MODE_FULLP, MODE_GRAD3, MODE_HVPQ); PWA_PAIR=0 switches it off
+bool pair_available(const pwa_handle* h, int mode);
+pwa_status pair_launch(pwa_handle* h, int mode, const double* theta, const double* v, const double* skip);
 // batch kernels (pwa_batch.cuh): kind 0 = K parameter sets (value only), 1 = K directions at the kept theta
 struct BatchArgs;
 typedef void (*batch_fn)(const LaneArgs, const BatchArgs);

@@ -45,12 +45,18 @@ lanes_fn PWA_CAT(lanes_kernel_h, PWA_LANES_H)(int combo, int mode) {
 }
 
 // two events per lane (pwa_sweep_pair.cuh): the fused sweep of the (4 x 8 slices) shape, H <= 2 (two events' G fit the registers)
-pair_fn PWA_CAT(pair_kernel_h, PWA_LANES_H)() {
+pair_fn PWA_CAT(pair_kernel_h, PWA_LANES_H)(int mode) {
 #if PWA_LANES_H <= 2
-  return lanes::k_sweep_pair<PWA_LANES_H>;
-#else
-  return nullptr;
+  switch (mode) {
+    case MODE_FULLP: return lanes::k_sweep_pair<PWA_LANES_H, MODE_FULLP>;
+    case MODE_GRAD3: return lanes::k_sweep_pair<PWA_LANES_H, MODE_GRAD3>;
+    case MODE_HVPQ: return lanes::k_sweep_pair<PWA_LANES_H, MODE_HVPQ>;
+    case MODE_GRAD: return lanes::k_sweep_pair<PWA_LANES_H, MODE_GRAD>;
+    case MODE_NLL: return lanes::k_sweep_pair<PWA_LANES_H, MODE_NLL>;
+  }
 #endif
+  (void)mode;
+  return nullptr;
 }
 
 // batch kernels (pwa_batch.cuh): only the warpgroup shapes (8 compute warps, 32-event tiles); kb: sets / directions per pass

@@ -30,13 +30,22 @@ namespace lanes {
 constexpr int KSP = 14;  // doubles of constants per resonance: the KS of the one-event kernel, lam2, 2 of padding (112-byte
                          // stride: the 8 slices of a warp read 8 different 16-byte bank groups)
 
-template <int H>
+// MODE: MODE_FULLP (P1, P2, Q1, Q2'), MODE_GRAD3 (P1, P2, P3: the gradient call of the split evaluation) or MODE_HVPQ
+// (Q1, Q2 at the kept theta: the cached HVP) - the three sweeps a Newton-CG fit and the timed fused call consist of.
+template <int H, int MODE>
 __global__ void __launch_bounds__(lanes_threads(8, 2), 1) k_sweep_pair(const __grid_constant__ LaneArgs a,
                                                                        const __grid_constant__ PairArgs pa) {
+  static_assert(MODE == MODE_FULLP || MODE == MODE_GRAD3 || MODE == MODE_HVPQ || MODE == MODE_GRAD || MODE == MODE_NLL,
+                "modes of the two-event kernel");
   constexpr int RHO = 4, LOG_SW = 3, NW = 8, TILE = 32;
   constexpr int SW = 1 << LOG_SW, EW = 32 / SW, NP = TILE / EW, NPP = NP / 2, RP = RHO * SW;
-  constexpr int NV = 4 * H;   // A_h, Adot_h (re, im) per event
-  constexpr int NACC = 8;     // P1, P2, Q1, Q2' per own resonance
+  constexpr bool WQ = MODE == MODE_FULLP || MODE == MODE_HVPQ;   // needs Adot, accumulates Q sums
+  constexpr bool WP = MODE == MODE_FULLP || MODE == MODE_GRAD3 || MODE == MODE_GRAD;  // accumulates P sums
+  constexpr bool BWD = MODE != MODE_NLL;
+  constexpr int NV = (WQ ? 4 : 2) * H;   // A_h [, Adot_h] (re, im) per event
+  constexpr int NACC = MODE == MODE_NLL ? 0 : vpr_of(MODE);  // FULLP: P1, P2, Q1, Q2'; GRAD3: P1, P2, P3; GRAD: P1, P2; HVPQ: Q1, Q2
+  constexpr int NA = NACC > 0 ? NACC : 1;
+  constexpr int QO = MODE == MODE_FULLP ? 4 : 0;
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   if (a.skip != nullptr && *a.skip != 0.0) return;
   const int lane = threadIdx.x & 31, w = (int)(threadIdx.x >> 5) - 4;
@@ -48,10 +57,13 @@ __global__ void __launch_bounds__(lanes_threads(8, 2), 1) k_sweep_pair(const __g
   for (int r = threadIdx.x; r < RP; r += blockDim.x) {
     double* k = Ks + r * KSP;
     if (r < R) {
-      resonance_constants(a.theta, a.v, r, (long long)a.off_mass + (long long)a.ch[r] * (TILE * 8), k);
-      const double M = a.theta[4 * r + 2], G = a.theta[4 * r + 3], vM = a.v[4 * r + 2], vG = a.v[4 * r + 3];
-      k[10] = 2.0 * (-2.0 * M * vM);        // lam2 = 2 lambda
-      k[11] = 2.0 * (G * vM + M * vG);
+      resonance_constants(a.theta, WQ ? a.v : nullptr, r, (long long)a.off_mass + (long long)a.ch[r] * (TILE * 8), k);
+      k[10] = k[11] = 0.0;
+      if (MODE == MODE_FULLP) {
+        const double M = a.theta[4 * r + 2], G = a.theta[4 * r + 3], vM = a.v[4 * r + 2], vG = a.v[4 * r + 3];
+        k[10] = 2.0 * (-2.0 * M * vM);        // lam2 = 2 lambda
+        k[11] = 2.0 * (G * vM + M * vG);
+      }
     } else {
       k[0] = 0.0; k[1] = 1.0; k[2] = 0.0; k[3] = __longlong_as_double((long long)a.off_mass);
       k[4] = k[5] = k[6] = k[7] = k[8] = k[9] = k[10] = k[11] = 0.0;
@@ -102,12 +114,12 @@ __global__ void __launch_bounds__(lanes_threads(8, 2), 1) k_sweep_pair(const __g
   // ======================================= compute warps ===================================================
   asm volatile("setmaxnreg.inc.sync.aligned.u32 240;");
   const int s = lane >> (5 - LOG_SW), e = lane & (EW - 1);
-  double acc[RHO][NACC];
+  double acc[RHO][NA];
   double s0 = 0.0, s1 = 0.0;
 #pragma unroll
   for (int j = 0; j < RHO; ++j)
 #pragma unroll
-    for (int q = 0; q < NACC; ++q) acc[j][q] = 0.0;
+    for (int q = 0; q < NA; ++q) acc[j][q] = 0.0;
   const double* lane_k = Ks + s * KSP;
   unsigned moff[RHO];
 #pragma unroll
@@ -141,39 +153,46 @@ __global__ void __launch_bounds__(lanes_threads(8, 2), 1) k_sweep_pair(const __g
       }
 
       // ---------------- forward, both events ----------------
-      double2 Gr[2][RHO][H], Br[2][RHO];
+      double2 Gr[2][BWD ? RHO : 1][H], Br[2][BWD ? RHO : 1];
       double x[2][NV];  // per event: slice partials A_h (re, im), then Adot_h (re, im)
 #pragma unroll
       for (int j = 0; j < RHO; ++j) {
         const double2* kk = reinterpret_cast<const double2*>(lane_k + j * (SW * KSP));
         const double2 k01 = kk[0];
         const double mg = lane_k[j * (SW * KSP) + 2];
-        const double2 c = kk[2], al = kk[3], be = kk[4];
+        const double2 c = kk[2], al = WQ ? kk[3] : make_double2(0.0, 0.0), be = WQ ? kk[4] : make_double2(0.0, 0.0);
 #pragma unroll
         for (int sd = 0; sd < 2; ++sd) {
           const double m = *reinterpret_cast<const double*>(sp + moff[j] + (sd ? evB : evA) * 8);
           const double xx = fma(-m, m, k01.x);
           const double u = fast_rcp(fma(xx, xx, k01.y));
           const double br = xx * u, bi = mg * u;
-          Br[sd][j] = make_double2(br, bi);
-          const double wr = fma(be.x, br, fma(-be.y, bi, al.x));  // zdot = (alpha + beta B) B
-          const double wi = fma(be.x, bi, fma(be.y, br, al.y));
+          if (BWD) Br[sd][j] = make_double2(br, bi);
+          double wr = 0.0, wi = 0.0;
+          if (WQ) {  // zdot = (alpha + beta B) B
+            wr = fma(be.x, br, fma(-be.y, bi, al.x));
+            wi = fma(be.x, bi, fma(be.y, br, al.y));
+          }
 #pragma unroll
           for (int h = 0; h < H; ++h) {
             const double2 F = *reinterpret_cast<const double2*>(sp + (sd ? fB : fA) + (j * SW * H + h) * (TILE * 16));
             const double gx = fma(br, F.x, -(bi * F.y)), gy = fma(br, F.y, bi * F.x);
-            Gr[sd][j][h] = make_double2(gx, gy);
+            if (BWD) Gr[sd][j][h] = make_double2(gx, gy);
             double* xs = x[sd];
             if (j == 0) {
               xs[2 * h] = fma(c.x, gx, -(c.y * gy));
               xs[2 * h + 1] = fma(c.x, gy, c.y * gx);
-              xs[2 * H + 2 * h] = fma(wr, gx, -(wi * gy));
-              xs[2 * H + 2 * h + 1] = fma(wr, gy, wi * gx);
+              if (WQ) {
+                xs[2 * H + 2 * h] = fma(wr, gx, -(wi * gy));
+                xs[2 * H + 2 * h + 1] = fma(wr, gy, wi * gx);
+              }
             } else {
               xs[2 * h] = fma(c.x, gx, fma(-c.y, gy, xs[2 * h]));
               xs[2 * h + 1] = fma(c.x, gy, fma(c.y, gx, xs[2 * h + 1]));
-              xs[2 * H + 2 * h] = fma(wr, gx, fma(-wi, gy, xs[2 * H + 2 * h]));
-              xs[2 * H + 2 * h + 1] = fma(wr, gy, fma(wi, gx, xs[2 * H + 2 * h + 1]));
+              if (WQ) {
+                xs[2 * H + 2 * h] = fma(wr, gx, fma(-wi, gy, xs[2 * H + 2 * h]));
+                xs[2 * H + 2 * h + 1] = fma(wr, gy, fma(wi, gx, xs[2 * H + 2 * h + 1]));
+              }
             }
           }
         }
@@ -216,52 +235,81 @@ __global__ void __launch_bounds__(lanes_threads(8, 2), 1) k_sweep_pair(const __g
           const double inv = 1.0 / Iv;
           const double om = wv * inv;
           if (count) {
-            s0 = fma(wv, log(Iv), s0);
+            if (MODE != MODE_HVPQ) s0 = fma(wv, log(Iv), s0);  // HVPQ: the scalars come from the kept gradient evaluation
             s1 += wv;
           }
-          double Idot = 0.0;
+          if (WQ) {
+            double Idot = 0.0;
 #pragma unroll
-          for (int h = 0; h < H; ++h)
-            Idot = fma(xs[2 * h], xs[2 * H + 2 * h], fma(xs[2 * h + 1], xs[2 * H + 2 * h + 1], Idot));
-          const double kap = 2.0 * Idot * inv;
+            for (int h = 0; h < H; ++h)
+              Idot = fma(xs[2 * h], xs[2 * H + 2 * h], fma(xs[2 * h + 1], xs[2 * H + 2 * h + 1], Idot));
+            const double kap = 2.0 * Idot * inv;
+#pragma unroll
+            for (int h = 0; h < H; ++h) {
+              xs[2 * H + 2 * h] = om * fma(-kap, xs[2 * h], xs[2 * H + 2 * h]);
+              xs[2 * H + 2 * h + 1] = om * fma(-kap, xs[2 * h + 1], xs[2 * H + 2 * h + 1]);
+            }
+          }
 #pragma unroll
           for (int h = 0; h < H; ++h) {
-            xs[2 * H + 2 * h] = om * fma(-kap, xs[2 * h], xs[2 * H + 2 * h]);
-            xs[2 * H + 2 * h + 1] = om * fma(-kap, xs[2 * h + 1], xs[2 * H + 2 * h + 1]);
             xs[2 * h] *= om;
             xs[2 * h + 1] *= om;
           }
         }
 #pragma unroll
-        for (int j = 0; j < RHO; ++j) {
+        for (int j = 0; j < (BWD ? RHO : 0); ++j) {
           const double br = Br[sd][j].x, bi = Br[sd][j].y;
-          const double2 l2 = *reinterpret_cast<const double2*>(lane_k + j * (SW * KSP) + 10);
-          double t1r, t1i, u1r, u1i;
-          {
+          double t1r = 0.0, t1i = 0.0, u1r = 0.0, u1i = 0.0;
+          if (WP) {  // t1 = B S = sum_h conj(omega A_h) G_h
             const double2 g = Gr[sd][j][0];
             t1r = fma(xs[0], g.x, xs[1] * g.y);
             t1i = fma(xs[0], g.y, -(xs[1] * g.x));
+#pragma unroll
+            for (int h = 1; h < H; ++h) {
+              const double2 gh = Gr[sd][j][h];
+              t1r = fma(xs[2 * h], gh.x, fma(xs[2 * h + 1], gh.y, t1r));
+              t1i = fma(xs[2 * h], gh.y, fma(-xs[2 * h + 1], gh.x, t1i));
+            }
+          }
+          if (WQ) {  // u1 = B S' = sum_h conj(omega (Adot_h - kappa A_h)) G_h
+            const double2 g = Gr[sd][j][0];
             u1r = fma(xs[2 * H], g.x, xs[2 * H + 1] * g.y);
             u1i = fma(xs[2 * H], g.y, -(xs[2 * H + 1] * g.x));
-          }
 #pragma unroll
-          for (int h = 1; h < H; ++h) {
-            const double2 g = Gr[sd][j][h];
-            t1r = fma(xs[2 * h], g.x, fma(xs[2 * h + 1], g.y, t1r));
-            t1i = fma(xs[2 * h], g.y, fma(-xs[2 * h + 1], g.x, t1i));
-            u1r = fma(xs[2 * H + 2 * h], g.x, fma(xs[2 * H + 2 * h + 1], g.y, u1r));
-            u1i = fma(xs[2 * H + 2 * h], g.y, fma(-xs[2 * H + 2 * h + 1], g.x, u1i));
+            for (int h = 1; h < H; ++h) {
+              const double2 gh = Gr[sd][j][h];
+              u1r = fma(xs[2 * H + 2 * h], gh.x, fma(xs[2 * H + 2 * h + 1], gh.y, u1r));
+              u1i = fma(xs[2 * H + 2 * h], gh.y, fma(-xs[2 * H + 2 * h + 1], gh.x, u1i));
+            }
           }
-          const double t2r = fma(br, t1r, -(bi * t1i)), t2i = fma(br, t1i, bi * t1r);  // B^2 S
-          acc[j][0] += t1r;  // P1
-          acc[j][1] += t1i;
-          acc[j][2] += t2r;  // P2
-          acc[j][3] += t2i;
-          acc[j][4] += u1r;  // Q1
-          acc[j][5] += u1i;
-          const double vr = fma(l2.x, t2r, fma(-l2.y, t2i, u1r)), vi = fma(l2.x, t2i, fma(l2.y, t2r, u1i));  // u1 + lam2 t2
-          acc[j][6] = fma(br, vr, fma(-bi, vi, acc[j][6]));  // Q2' = Q2 + lam2 P3
-          acc[j][7] = fma(br, vi, fma(bi, vr, acc[j][7]));
+          if (MODE == MODE_GRAD) {
+            acc[j][0] += t1r;  // P1
+            acc[j][1] += t1i;
+            acc[j][2] = fma(br, t1r, fma(-bi, t1i, acc[j][2]));  // P2
+            acc[j][3] = fma(br, t1i, fma(bi, t1r, acc[j][3]));
+          } else if (WP) {
+            const double t2r = fma(br, t1r, -(bi * t1i)), t2i = fma(br, t1i, bi * t1r);  // B^2 S
+            acc[j][0] += t1r;  // P1
+            acc[j][1] += t1i;
+            acc[j][2] += t2r;  // P2
+            acc[j][3] += t2i;
+            if (MODE == MODE_GRAD3) {
+              acc[j][4] = fma(br, t2r, fma(-bi, t2i, acc[j][4]));  // P3
+              acc[j][5] = fma(br, t2i, fma(bi, t2r, acc[j][5]));
+            } else {  // FULLP: u1 <- u1 + lam2 t2, so that the Q2 accumulation below gives Q2' = Q2 + lam2 P3
+              const double2 l2 = *reinterpret_cast<const double2*>(lane_k + j * (SW * KSP) + 10);
+              const double vr = fma(l2.x, t2r, fma(-l2.y, t2i, u1r)), vi = fma(l2.x, t2i, fma(l2.y, t2r, u1i));
+              acc[j][QO] += u1r;  // Q1 (before the fold)
+              acc[j][QO + 1] += u1i;
+              acc[j][QO + 2] = fma(br, vr, fma(-bi, vi, acc[j][QO + 2]));
+              acc[j][QO + 3] = fma(br, vi, fma(bi, vr, acc[j][QO + 3]));
+            }
+          } else {  // HVPQ
+            acc[j][0] += u1r;  // Q1
+            acc[j][1] += u1i;
+            acc[j][2] = fma(br, u1r, fma(-bi, u1i, acc[j][2]));  // Q2
+            acc[j][3] = fma(br, u1i, fma(bi, u1r, acc[j][3]));
+          }
         }
       }
       t += NW / NPP;
