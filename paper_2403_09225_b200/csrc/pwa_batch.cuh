@@ -52,7 +52,7 @@ __global__ void __launch_bounds__(lanes_threads(NW, 2), 1) k_batch_lanes(const _
   constexpr int NS0 = KIND == BK_NLL ? KB : 1;
   // PAIR (value batch, 8 slices x 4 events): a warp takes TWO columns of every second tile and a lane two events, one per
   // column, odd slices in the opposite order - see the compute section
-  constexpr bool PAIR = KIND == BK_NLL && LOG_SW == 3 && NW == NP && KB >= 4;
+  constexpr bool PAIR = KIND == BK_NLL && LOG_SW == 3 && NW == NP;
   static_assert(NW % NP == 0, "a warp keeps its column");
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   const int lane = threadIdx.x & 31, w = (int)(threadIdx.x >> 5) - 4;  // w: compute-warp index (warps 0..3: producer group)
