@@ -58,8 +58,15 @@ pwa_status pair_launch(pwa_handle* h, int mode, const double* theta, const doubl
   PairArgs p;
   size_t smem = 0;
   if (!fn || !pair_plan(h, p, smem)) return set_error(h, PWA_ERR_INVALID_ARG, "no two-event kernel for this shape", cudaSuccess);
-  cudaError_t ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (ce != cudaSuccess) return set_error(h, PWA_ERR_CUDA, "cudaFuncSetAttribute(two-event sweep)", ce);
+  cudaError_t ce = cudaSuccess;
+  if (!(h->attr_done & (1u << mode))) {  // once per handle and mode, not per launch
+    // the attribute belongs to the FUNCTION, shared by every handle of the process: always raise it to the device limit
+    int dev_smem = 0;
+    cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device);
+    ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, dev_smem);
+    if (ce != cudaSuccess) return set_error(h, PWA_ERR_CUDA, "cudaFuncSetAttribute(two-event sweep)", ce);
+    h->attr_done |= 1u << mode;
+  }
   LaneArgs a = h->largs;
   a.theta = theta;
   a.v = v;
@@ -137,8 +144,15 @@ pwa_status batch_launch(pwa_handle* h, int kind, int kb, const double* theta, co
     }
     h->batch_doubles = need;
   }
-  cudaError_t ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (ce != cudaSuccess) return set_error(h, PWA_ERR_CUDA, "cudaFuncSetAttribute(batch sweep)", ce);
+  cudaError_t ce = cudaSuccess;
+  const unsigned abit = 1u << (8 + 4 * kind + (kb - 1));
+  if (!(h->attr_done & abit)) {
+    int dev_smem = 0;  // function-wide attribute: the device limit, whatever this handle needs
+    cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device);
+    ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, dev_smem);
+    if (ce != cudaSuccess) return set_error(h, PWA_ERR_CUDA, "cudaFuncSetAttribute(batch sweep)", ce);
+    h->attr_done |= abit;
+  }
   b.theta = theta;
   b.v = v;
   b.partial = h->d_batch;

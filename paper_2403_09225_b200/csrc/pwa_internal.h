@@ -64,6 +64,7 @@ struct pwa_handle {
   double* d_io = nullptr;   // theta | v | nll | grad | hv   (1 + 4P doubles, padded)
   double* h_pin = nullptr;  // pinned host mirror of d_io
   double* d_fit = nullptr;  // fit vectors
+  unsigned attr_done = 0;          // bit per kernel whose shared-memory attribute this handle has already set (pair modes 0..5, batch 8..)
   double* d_batch = nullptr;       // batch sweeps: per-block partial rows, column sums, one raw vector
   size_t batch_doubles = 0;
   double* h_fit = nullptr;  // pinned scalars of the fit driver
