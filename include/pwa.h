@@ -19,7 +19,8 @@
  * F_rh(i) ("amp") is the parameter-free projection of PAPER.md:70, an input computed once by the caller.
  *
  * Conventions
- *   - Every call returns a pwa_status; nothing throws across this boundary; no global state.  One handle = one device
+ *   - Every call returns a pwa_status; nothing throws across this boundary; no global state (one exception: the scratch
+ *     array of pwa_nll_grad_hvp_static).  One handle = one device
  *     + one stream; a handle is not thread-safe, different handles are independent.  Every call binds the calling
  *     thread to the handle's device for its duration and restores the caller's current device before it returns, so
  *     a handle may be used from any host thread (one thread per GPU).
@@ -226,6 +227,35 @@ pwa_status pwa_fit_newton_cg(pwa_handle* h, double* theta_inout, const pwa_fit_o
  * nll_host 1 double, grad_host / hv_host P doubles in HOST memory (each may be NULL). */
 pwa_status pwa_nll_grad_hvp_host(pwa_handle* h, const double* theta_host, const double* v_host,
                                  double* nll_host, double* grad_host, double* hv_host);
+
+/* ---- allocation-free evaluation (no handle) ------------------------------------------------------
+ * For callers that cannot allocate device memory: code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc.  pwa_create allocates a handle's scratch; this ONE entry point needs no handle and calls no
+ * cudaMalloc, cudaFree or allocating library routine: its scratch (per-resonance constants, per-block partial sums of
+ * Eqs. 4-7, their column sums, the raw vector, the reduction's ticket) lives in a fixed
+ * PWA_STATIC_SCRATCH_BYTES array in the library's device image, which every GPU that loads the library holds until
+ * the process exits.  Same result as pwa_nll_grad_hvp on a handle created from the same descriptor (Eq. 3,
+ * :90 Eq. 6, :95 Eq. 7) to rounding: the sweep is the event-per-thread kernel of csrc/pwa_kernels.cuh (the generic
+ * variant), another summation tree than the tiled kernels; bit-identical between repeated calls on one device.
+ *   model   as for pwa_create with mem = PWA_MEM_DEVICE: the event buffers are DEVICE pointers, read in place (borrow
+ *           is ignored; amp 16-byte aligned, mass / weight 8-byte aligned); res_chan is a HOST pointer read during the
+ *           call (passed to the kernels by value); model->stream is the stream the work is enqueued on.
+ *   theta, v, nll, grad, hv   DEVICE pointers as for pwa_nll_grad_hvp, P = 4 n_res.  v may be NULL (then hv must be
+ *           NULL); each of nll, grad, hv may be NULL (not wanted), not all three.  Outputs may not alias inputs.
+ * Limits: n_res <= PWA_STATIC_MAX_RES (the partial rows of more resonances do not fit the fixed array), n_hel and
+ * n_chan as for pwa_create, any number of events.  Beyond them: PWA_ERR_INVALID_ARG, message in pwa_last_error(NULL).
+ * Enqueues three kernels and returns without synchronising.  The first call on each device also looks up the array's
+ * device address and the launch configuration (host-side queries, no allocation by this library; the CUDA runtime
+ * loads the kernels on their first launch): under graph capture make one call with the same n_res / n_hel before the
+ * capture starts.
+ * EVERY call on a device shares the one array, which keeps the previous call's contents (what must start at zero -
+ * the reduction's ticket, the non-finite flag - is cleared by the call's first kernel).  Calls that overlap on the
+ * GPU - two streams, or two host threads on different streams - race on it and give wrong results: order them on one
+ * stream or with events.  The array holds no result a later call reads. */
+#define PWA_STATIC_MAX_RES 64
+#define PWA_STATIC_SCRATCH_BYTES (4u << 20) /* 4 MiB per device */
+pwa_status pwa_nll_grad_hvp_static(const pwa_model_desc* model, const double* theta, const double* v, double* nll,
+                                   double* grad, double* hv);
 
 /* ---- fit fractions (Table 1 of the paper lists a "fraction" F_i per resonance; S20) ----
  * frac[r] = sum_mc sum_h |c_r B_r(j) F_rh(j)|^2 / sum_mc I_j  over the handle's phase-space MC sample.

@@ -16,7 +16,7 @@ from typing import Optional
 
 __all__ = ["PwaError", "lib_path", "load", "pwa_create", "pwa_create_rich", "pwa_rich_desc", "PWA_LS_CONST", "PWA_LS_MASSDEP", "PWA_LS_FLATTE", "pwa_destroy", "pwa_n_params", "pwa_raw_size", "pwa_nll",
            "pwa_nll_grad", "pwa_hvp", "pwa_nll_grad_hvp", "pwa_raw_sums", "pwa_combine", "pwa_fit_opts",
-           "pwa_fit_result", "pwa_fit_opts_default", "pwa_fit_newton_cg", "pwa_nll_grad_hvp_host", "pwa_fit_fractions",
+           "pwa_fit_result", "pwa_fit_opts_default", "pwa_fit_newton_cg", "pwa_nll_grad_hvp_host", "pwa_nll_grad_hvp_static", "pwa_fit_fractions",
            "pwa_nll_grad_for_hvp", "pwa_hvp_cached", "pwa_nll_batch", "pwa_hvp_cached_batch", "pwa_hessian",
            "pwa_status_flags", "pwa_profile_enable", "pwa_profile_read", "pwa_kernel_launches", "pwa_bytes_per_eval",
            "pwa_kernel_variant", "pwa_last_error", "pwa_version", "Model", "STATUS_NAMES", "EXPORTS"]
@@ -33,7 +33,7 @@ PWA_LS_CONST, PWA_LS_MASSDEP, PWA_LS_FLATTE = 0, 1, 2
 # every symbol include/pwa.h declares
 EXPORTS = ["pwa_create", "pwa_create_rich", "pwa_destroy", "pwa_n_params", "pwa_nll", "pwa_nll_grad", "pwa_hvp", "pwa_nll_grad_hvp",
            "pwa_raw_size", "pwa_raw_sums", "pwa_combine", "pwa_fit_opts_default", "pwa_fit_newton_cg",
-           "pwa_nll_grad_hvp_host", "pwa_fit_fractions", "pwa_nll_grad_for_hvp", "pwa_hvp_cached", "pwa_nll_batch", "pwa_hvp_cached_batch", "pwa_hessian",
+           "pwa_nll_grad_hvp_host", "pwa_nll_grad_hvp_static", "pwa_fit_fractions", "pwa_nll_grad_for_hvp", "pwa_hvp_cached", "pwa_nll_batch", "pwa_hvp_cached_batch", "pwa_hessian",
            "pwa_status_flags", "pwa_profile_enable", "pwa_profile_read",
            "pwa_kernel_launches", "pwa_bytes_per_eval", "pwa_kernel_variant", "pwa_last_error", "pwa_version"]
 
@@ -106,6 +106,7 @@ def load():
     lib.pwa_fit_opts_default.restype = None
     lib.pwa_fit_newton_cg.argtypes = [vp, dp, POINTER(pwa_fit_opts), POINTER(pwa_fit_result)]
     lib.pwa_nll_grad_hvp_host.argtypes = [vp, dp, dp, dp, dp, dp]
+    lib.pwa_nll_grad_hvp_static.argtypes = [POINTER(pwa_model_desc), dp, dp, dp, dp, dp]
     lib.pwa_fit_fractions.argtypes = [vp, dp, dp]
     lib.pwa_nll_grad_for_hvp.argtypes = [vp, dp, dp, dp]
     lib.pwa_hvp_cached.argtypes = [vp, dp, dp]
@@ -288,6 +289,36 @@ def pwa_nll_grad_hvp_host(h, theta_host, v_host, nll_host, grad_host, hv_host) -
     """Host-buffer entry point: numpy float64 arrays (or CPU tensors); copies in, evaluates, copies out, syncs."""
     _check(load().pwa_nll_grad_hvp_host(h, _ptr(theta_host), _ptr(v_host), _ptr(nll_host), _ptr(grad_host),
                                         _ptr(hv_host)), h)
+
+
+PWA_STATIC_MAX_RES = 64
+
+
+def pwa_nll_grad_hvp_static(res_chan, data_mass, data_amp, data_weight, mc_mass, mc_amp, theta, v, nll, grad, hv, *,
+                            device: int = 0, stream: int = 0) -> None:
+    """pwa_nll_grad_hvp_static of include/pwa.h: the fused evaluation without a handle and without any device
+    allocation (fixed scratch array inside the library; n_res <= PWA_STATIC_MAX_RES; calls that overlap on the GPU
+    race).  Event buffers: contiguous CUDA float64 tensors in the layouts of pwa_create, read in place; res_chan [R]
+    int32 on the CPU; theta, v, nll, grad, hv: CUDA float64 tensors (v, nll, grad, hv may each be None)."""
+    import torch
+    R, H, C = int(mc_amp.shape[0]), int(mc_amp.shape[1]), int(mc_mass.shape[0])
+    for t in [data_mass, data_amp, mc_mass, mc_amp] + ([data_weight] if data_weight is not None else []):
+        if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+            raise TypeError("event buffers must be contiguous CUDA float64 tensors")
+    rc = torch.as_tensor(res_chan).to(torch.int32).cpu().contiguous()
+    if rc.numel() != R:
+        raise ValueError("res_chan must have one entry per resonance")
+    d = pwa_model_desc()
+    d.n_res, d.n_hel, d.n_chan = R, H, C
+    d.res_chan = rc.data_ptr()
+    d.data = pwa_sample(int(data_mass.shape[1]), 0, data_mass.data_ptr(), data_amp.data_ptr(),
+                        None if data_weight is None else data_weight.data_ptr())
+    d.mc = pwa_sample(int(mc_mass.shape[1]), 0, mc_mass.data_ptr(), mc_amp.data_ptr(), None)
+    d.mem, d.borrow, d.device, d.stream = PWA_MEM_DEVICE, 1, device, stream or None
+    P = 4 * R
+    opt = lambda t, n, name: None if t is None else _dev_f64(t, n, name)
+    _check(load().pwa_nll_grad_hvp_static(byref(d), _dev_f64(theta, P, "theta"), opt(v, P, "v"), opt(nll, 1, "nll"),
+                                          opt(grad, P, "grad"), opt(hv, P, "hv")))
 
 
 def pwa_nll_grad_for_hvp(h, theta, nll, grad) -> None:

@@ -18,7 +18,7 @@ CSRC = os.path.join(PKG, "csrc")
 OBJ = os.path.join(PKG, "build")
 LIB = os.path.join(PKG, "libpwa_b200.so")
 # (source, object name, extra defines)
-UNITS = [("pwa_api.cu", "pwa_api.o", []), ("pwa_fit.cu", "pwa_fit.o", []), ("pwa_fractions.cu", "pwa_fractions.o", []), ("pwa_sweep_lanes.cu", "pwa_sweep_lanes.o", []), ("pwa_batch.cu", "pwa_batch.o", [])] + \
+UNITS = [("pwa_api.cu", "pwa_api.o", []), ("pwa_fit.cu", "pwa_fit.o", []), ("pwa_fractions.cu", "pwa_fractions.o", []), ("pwa_sweep_lanes.cu", "pwa_sweep_lanes.o", []), ("pwa_batch.cu", "pwa_batch.o", []), ("pwa_static.cu", "pwa_static.o", [])] + \
         [("pwa_sweep_lanes_inst.cu", f"pwa_sweep_lanes_h{h}.o", [f"-DPWA_LANES_H={h}"]) for h in (1, 2, 3, 4)]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 CFLAGS = [*ARCH, "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC,-O2"]
