@@ -347,6 +347,9 @@ def main():
     ap.add_argument("--batch", type=int, default=4, help="--mode nll_batch / hvp_cached_batch: evaluations per call (K)")
     ap.add_argument("--sustained-seconds", type=float, default=1.2,
                     help="length of the back-to-back run behind roofline_sustained (0 = skip)")
+    ap.add_argument("--store", default="auto", choices=["auto", "borrow", "copy"],
+                    help="event store of the handle: borrow = the workload's planes in place (zero copy); copy = a library-owned "
+                         "copy, which shapes that need 8-event tiles keep TILED (one bulk copy per stage); auto = copy for config 4")
     ap.add_argument("--csrc-digest", action="store_true", help="print the digest a profiles/*_traffic.csv row must carry, and exit")
     args = ap.parse_args()
     if args.csrc_digest:
@@ -387,7 +390,10 @@ def main():
     w = workloads.make_workload(cfg, dev)
     torch.cuda.synchronize()
     t_gen = time.time() - t_gen
-    m = pwa.Model(w, device=local, borrow=True)
+    store = args.store if args.store != "auto" else ("copy" if args.config == 4 else "borrow")
+    if store == "copy":
+        torch.cuda.empty_cache()  # the library's copy is allocated beside the workload (config 4: 2 x 70.7 GB of 180 GB)
+    m = pwa.Model(w, device=local, borrow=store == "borrow")
     P = m.P
     th_np = workloads.random_start(base, 0).numpy()
     v_np = workloads.direction(base, 0).numpy()
@@ -556,6 +562,7 @@ def main():
         "config": {"workload": f"config {args.config} ({cfg.name}): R={cfg.n_res} H={cfg.n_hel} C={cfg.n_chan} "
                                f"P={cfg.n_par}, N_mc={cfg.n_mc} N_data={cfg.n_data} per GPU"
                                f"{', weighted data' if cfg.weighted else ''}",
+                   "store": "borrowed planes (zero copy)" if store == "borrow" else "library-owned copy",
                    "l2": f"inputs ({bytes_per_step / 1e6:.0f} MB per step) exceed the 126 MB L2; no flush needed"
                          if bytes_per_step > 2 * 126e6 else "inputs fit in L2 (cache-resident case)",
                    "kernel_variant": pwa.pwa_kernel_variant(m.h), "parallelism": f"event shards x{world}",

@@ -354,6 +354,91 @@ static pwa_status store_sample(pwa_handle* h, const pwa_model_desc* m, const pwa
   return PWA_OK;
 }
 
+// Planes -> tiled store (TiledDev, pwa_common.cuh).  The source holds `cnt` events starting at event i0 (a multiple of
+// 32) of the sample, planes `stride` events apart; a warp moves one plane row of a 32-event group at a time (512
+// contiguous bytes in, four 128-byte tile rows out).  Events from i0 + cnt to the end of their last tile are zeroed.
+static __global__ void __launch_bounds__(256) k_retile(const double2* __restrict__ amp, const double* __restrict__ mass,
+                                                       const double* __restrict__ weight, long long i0, long long cnt,
+                                                       long long stride, int R, int C, TiledDev t, unsigned char* dst) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+  const long long groups = (cnt + 31) / 32, cap = (t.n + 7) / 8 * 8;
+  for (long long g = blockIdx.x; g < groups; g += gridDim.x) {
+    const long long k = g * 32 + lane, i = i0 + k;  // source-local and sample-wide event index
+    if (i >= cap) continue;
+    const bool valid = k < cnt;
+    const int rows = R * t.H;
+    for (int row = warp; row < rows + C + 1; row += nwarp) {
+      if (row < rows) {
+        const double2 f = valid ? amp[(size_t)row * stride + k] : make_double2(0.0, 0.0);
+        *reinterpret_cast<double2*>(dst + tiled_amp_off(t, row / t.H, row % t.H, i)) = f;
+      } else if (row < rows + C) {
+        const int c = row - rows;
+        *reinterpret_cast<double*>(dst + tiled_mass_off(t, c, i)) = valid ? mass[(size_t)c * stride + k] : 0.0;
+      } else {
+        *reinterpret_cast<double*>(dst + tiled_weight_off(t, i)) = (valid && weight) ? weight[k] : 0.0;
+      }
+    }
+  }
+}
+
+// Builds the tiled store of one sample (h->tstore[which], layout already filled in) from the caller's planes.
+static pwa_status store_sample_tiled(pwa_handle* h, const pwa_model_desc* m, const pwa_sample& s, int which, void** own) {
+  const long long n = s.n_events, sin = s.stride ? s.stride : s.n_events;
+  const int R = m->n_res, H = m->n_hel, C = m->n_chan, planes = R * H;
+  TiledDev& t = h->tstore[which];
+  t.n = n;
+  t.weighted = s.weight != nullptr;
+  h->smp[which].n = n;
+  h->smp[which].stride = 0;
+  h->smp[which].mass = nullptr;
+  h->smp[which].amp = nullptr;
+  h->smp[which].weight = nullptr;
+  const size_t bytes = (size_t)((n + 7) / 8) * t.tile_bytes;
+  unsigned char* dst = nullptr;
+  if (cudaMalloc(&dst, bytes) != cudaSuccess) {
+    cudaGetLastError();
+    return set_error(nullptr, PWA_ERR_OOM, "device allocation of the (tiled) event store failed", cudaSuccess);
+  }
+  own[0] = dst;
+  t.base = dst;
+  const int grid = 8 * h->num_sms;
+  if (m->mem == PWA_MEM_DEVICE) {
+    k_retile<<<grid, 256, 0, h->stream>>>(reinterpret_cast<const double2*>(s.amp), s.mass, s.weight, 0, n, sin, R, C, t, dst);
+    PWA_CUDA_CHECK(nullptr, cudaGetLastError());
+    PWA_CUDA_CHECK(nullptr, cudaStreamSynchronize(h->stream));  // the caller may free its buffers when pwa_create returns
+    return PWA_OK;
+  }
+  // host planes: staged through a device buffer of E events per plane (about 256 MB), chunk by chunk
+  const size_t per_event = (size_t)planes * 16 + (size_t)C * 8 + 8;
+  long long E = (long long)((256u << 20) / per_event) / 32 * 32;
+  E = std::max<long long>(32, std::min<long long>(E, round_up(n, 32)));
+  double *ta = nullptr, *tm = nullptr, *tw = nullptr;
+  if (cudaMalloc(&ta, (size_t)planes * E * 16) != cudaSuccess || cudaMalloc(&tm, (size_t)C * E * 8) != cudaSuccess ||
+      cudaMalloc(&tw, (size_t)E * 8) != cudaSuccess) {
+    cudaGetLastError();
+    if (ta) cudaFree(ta);
+    if (tm) cudaFree(tm);
+    return set_error(nullptr, PWA_ERR_OOM, "device allocation of the staging buffers failed", cudaSuccess);
+  }
+  cudaError_t ce = cudaSuccess;
+  for (long long i0 = 0; i0 < n && ce == cudaSuccess; i0 += E) {
+    const long long cnt = std::min(E, n - i0);
+    ce = cudaMemcpy2DAsync(ta, (size_t)E * 16, s.amp + (size_t)i0 * 2, (size_t)sin * 16, (size_t)cnt * 16, planes, cudaMemcpyHostToDevice, h->stream);
+    if (ce == cudaSuccess)
+      ce = cudaMemcpy2DAsync(tm, (size_t)E * 8, s.mass + i0, (size_t)sin * 8, (size_t)cnt * 8, C, cudaMemcpyHostToDevice, h->stream);
+    if (ce == cudaSuccess && s.weight) ce = cudaMemcpyAsync(tw, s.weight + i0, (size_t)cnt * 8, cudaMemcpyHostToDevice, h->stream);
+    if (ce != cudaSuccess) break;
+    k_retile<<<grid, 256, 0, h->stream>>>(reinterpret_cast<const double2*>(ta), tm, s.weight ? tw : nullptr, i0, cnt, E, R, C, t, dst);
+    ce = cudaGetLastError();
+  }
+  if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
+  cudaFree(ta);
+  cudaFree(tm);
+  cudaFree(tw);
+  if (ce != cudaSuccess) return set_error(nullptr, PWA_ERR_CUDA, "upload of the (tiled) event store", ce);
+  return PWA_OK;
+}
+
 extern "C" pwa_status pwa_create(const pwa_model_desc* m, pwa_handle** out) { return pwa_create_rich(m, nullptr, out); }
 
 extern "C" pwa_status pwa_create_rich(const pwa_model_desc* m, const pwa_rich_desc* rich, pwa_handle** out) {
@@ -423,8 +508,28 @@ extern "C" pwa_status pwa_create_rich(const pwa_model_desc* m, const pwa_rich_de
   h->weighted = m->data.weight != nullptr;
   cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, m->device);
 
-  pwa_status st = store_sample(h, m, m->mc, 0, h->owned);
-  if (st == PWA_OK) st = store_sample(h, m, m->data, 1, h->owned + 3);
+  // Copy-mode handles of shapes that need 8-event tiles keep the events tiled (one bulk copy per stage instead of
+  // tensor copies of 128-byte rows: pwa_sweep_lanes.cuh, PROD 4)
+  const char* force = std::getenv("PWA_VARIANT");
+  const bool want_lanes = (!force || std::strcmp(force, "lanes") == 0) && !rich_kernel;
+  if (want_lanes && !rich && !m->borrow && m->data.n_events < (1LL << 30) && m->mc.n_events < (1LL << 30) &&
+      !(m->mem == PWA_MEM_DEVICE && (((uintptr_t)m->data.amp | (uintptr_t)m->mc.amp) & 15))) {
+    int phase_mul = 0;
+    unsigned tile_bytes = 0, off_mass = 0, off_wgt = 0;
+    if (lanes_wants_tiled(m->device, m->n_res, m->n_hel, m->n_chan, &phase_mul, &tile_bytes, &off_mass, &off_wgt)) {
+      h->tiled = true;
+      for (int k = 0; k < 2; ++k) {
+        h->tstore[k].base = nullptr;
+        h->tstore[k].tile_bytes = tile_bytes;
+        h->tstore[k].off_mass = off_mass;
+        h->tstore[k].off_wgt = off_wgt;
+        h->tstore[k].H = m->n_hel;
+        h->tstore[k].phase_mul = phase_mul;
+      }
+    }
+  }
+  pwa_status st = h->tiled ? store_sample_tiled(h, m, m->mc, 0, h->owned) : store_sample(h, m, m->mc, 0, h->owned);
+  if (st == PWA_OK) st = h->tiled ? store_sample_tiled(h, m, m->data, 1, h->owned + 3) : store_sample(h, m, m->data, 1, h->owned + 3);
   if (st != PWA_OK) {
     std::string msg;
     { std::lock_guard<std::mutex> lk(g_err_mutex); msg = g_create_err; }
@@ -440,12 +545,11 @@ extern "C" pwa_status pwa_create_rich(const pwa_model_desc* m, const pwa_rich_de
   }
   why.clear();
   h->weight_padded = h->owned[5] != nullptr;
-  const char* force = std::getenv("PWA_VARIANT");
-  const bool want_lanes = (!force || std::strcmp(force, "lanes") == 0) && !rich_kernel;
   if (want_lanes) {
     st = lanes_configure(h, why);
     if (st != PWA_OK) return fail_create(h, st, h->err);
   }
+  if (h->tiled && h->variant == 0) return fail_create(h, PWA_ERR_CUDA, "the tiled event store needs the lanes kernel (internal): " + why);
   if (h->variant == 0 && force) why = std::string("PWA_VARIANT=") + force + (why.empty() ? "" : "; " + why);
   if (h->variant == 0) {
     int block = 256;

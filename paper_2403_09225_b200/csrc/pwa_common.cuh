@@ -41,6 +41,31 @@ struct SampleDev {
   long long n, stride;
 };
 
+// Library-owned TILED event store (copy-mode handles whose shape needs 8-event tiles, e.g. R = 100, H = 4): tile t holds
+// the events 8t .. 8t+7 in ONE contiguous block of tile_bytes, laid out exactly as a stage of the sweep's ring -
+//   [resonance r][helicity h][8 events x (re, im)]  128-byte rows, the 16-byte chunk of event e at position e ^ phase(r),
+//                                                   phase(r) = (r * phase_mul) & 7   (bank-conflict-free reads)
+//   [channel c][8 events]                           masses, at off_mass
+//   [8 events]                                      weights (zeros when the sample has none), at off_wgt
+// so that one bulk copy (cp.async.bulk) of contiguous HBM fills a stage.  Events beyond n are zero.
+struct TiledDev {
+  const unsigned char* base;
+  long long n;
+  unsigned tile_bytes, off_mass, off_wgt;
+  int H, phase_mul;
+  bool weighted;
+};
+__host__ __device__ inline size_t tiled_amp_off(const TiledDev& t, int r, int h, long long i) {
+  const unsigned e = (unsigned)(i & 7), ph = (unsigned)(r * t.phase_mul) & 7u;
+  return (size_t)(i >> 3) * t.tile_bytes + ((size_t)r * t.H + h) * 128 + ((e ^ ph) << 4);
+}
+__host__ __device__ inline size_t tiled_mass_off(const TiledDev& t, int c, long long i) {
+  return (size_t)(i >> 3) * t.tile_bytes + t.off_mass + (size_t)c * 64 + ((size_t)(i & 7) << 3);
+}
+__host__ __device__ inline size_t tiled_weight_off(const TiledDev& t, long long i) {
+  return (size_t)(i >> 3) * t.tile_bytes + t.off_wgt + ((size_t)(i & 7) << 3);
+}
+
 struct SweepArgs {
   SampleDev s[2];        // 0 = MC, 1 = data
   const double* K;       // [R][KSTRIDE]

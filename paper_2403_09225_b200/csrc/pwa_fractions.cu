@@ -11,9 +11,11 @@ namespace {
 
 constexpr int FB = 256;  // threads per block
 
-template <int H>
-__global__ void __launch_bounds__(FB) k_fractions(SampleDev s, const int* __restrict__ ch, const double* __restrict__ theta,
-                                                  int R, double* __restrict__ partial /* [grid][R + 1] */) {
+// TILED: the handle keeps its events as 8-event tiles (TiledDev, pwa_common.cuh): same pass, other addresses
+template <int H, bool TILED>
+__global__ void __launch_bounds__(FB) k_fractions(SampleDev s, TiledDev td, const int* __restrict__ ch,
+                                                  const double* __restrict__ theta, int R,
+                                                  double* __restrict__ partial /* [grid][R + 1] */) {
   extern __shared__ double sm[];  // [R][4] constants (M^2, (M Gamma)^2, c_re, c_im; M Gamma kept in k[1] as a square root
                                   // would cost precision, so a fifth value) then [FB/32][R + 1] warp sums
   double* K = sm;                 // [R][5]
@@ -32,7 +34,7 @@ __global__ void __launch_bounds__(FB) k_fractions(SampleDev s, const int* __rest
   for (int k = threadIdx.x; k < (FB / 32) * (R + 1); k += FB) acc[k] = 0.0;
   __syncthreads();
   double* mine = acc + w * (R + 1);
-  const long long n = s.n, stride = s.stride;
+  const long long n = TILED ? td.n : s.n, stride = s.stride;
   const long long nwarp_iters = (n + 31) / 32;
   for (long long it = (long long)blockIdx.x * (FB / 32) + w; it < nwarp_iters; it += (long long)gridDim.x * (FB / 32)) {
     const long long i = it * 32 + lane;
@@ -42,7 +44,8 @@ __global__ void __launch_bounds__(FB) k_fractions(SampleDev s, const int* __rest
 #pragma unroll
     for (int h = 0; h < H; ++h) Ar[h] = Ai[h] = 0.0;
     for (int r = 0; r < R; ++r) {
-      const double m = s.mass[(long long)ch[r] * stride + ii];
+      const double m = TILED ? *reinterpret_cast<const double*>(td.base + tiled_mass_off(td, ch[r], ii))
+                             : s.mass[(long long)ch[r] * stride + ii];
       const double xx = K[5 * r] - m * m;
       const double inv = 1.0 / (xx * xx + K[5 * r + 1]);
       const double br = xx * inv, bi = K[5 * r + 2] * inv;  // B = conj(D) / |D|^2
@@ -50,7 +53,8 @@ __global__ void __launch_bounds__(FB) k_fractions(SampleDev s, const int* __rest
       double own = 0.0;
 #pragma unroll
       for (int h = 0; h < H; ++h) {
-        const double2 F = s.amp[((long long)r * H + h) * stride + ii];
+        const double2 F = TILED ? *reinterpret_cast<const double2*>(td.base + tiled_amp_off(td, r, h, ii))
+                                : s.amp[((long long)r * H + h) * stride + ii];
         const double tr = zr * F.x - zi * F.y, ti = zr * F.y + zi * F.x;
         Ar[h] += tr;
         Ai[h] += ti;
@@ -176,17 +180,26 @@ frac_rich_fn frac_rich_kernel(int H) {
   return nullptr;
 }
 
-typedef void (*frac_fn)(SampleDev, const int*, const double*, int, double*);
-frac_fn frac_kernel(int H) {
+typedef void (*frac_fn)(SampleDev, TiledDev, const int*, const double*, int, double*);
+frac_fn frac_kernel(int H, bool tiled) {
+  if (tiled) {  // tiled stores exist for the shapes of the lanes sweep only (n_hel <= 4)
+    switch (H) {
+      case 1: return k_fractions<1, true>;
+      case 2: return k_fractions<2, true>;
+      case 3: return k_fractions<3, true>;
+      case 4: return k_fractions<4, true>;
+    }
+    return nullptr;
+  }
   switch (H) {
-    case 1: return k_fractions<1>;
-    case 2: return k_fractions<2>;
-    case 3: return k_fractions<3>;
-    case 4: return k_fractions<4>;
-    case 5: return k_fractions<5>;
-    case 6: return k_fractions<6>;
-    case 7: return k_fractions<7>;
-    case 8: return k_fractions<8>;
+    case 1: return k_fractions<1, false>;
+    case 2: return k_fractions<2, false>;
+    case 3: return k_fractions<3, false>;
+    case 4: return k_fractions<4, false>;
+    case 5: return k_fractions<5, false>;
+    case 6: return k_fractions<6, false>;
+    case 7: return k_fractions<7, false>;
+    case 8: return k_fractions<8, false>;
   }
   return nullptr;
 }
@@ -220,7 +233,7 @@ extern "C" pwa_status pwa_fit_fractions(pwa_handle* h, const double* theta, doub
     if (cudaError_t ce = cudaGetLastError()) return set_error(h, PWA_ERR_CUDA, "launch k_fractions_final", ce);
     return PWA_OK;
   }
-  frac_fn fn = frac_kernel(h->n_hel);
+  frac_fn fn = frac_kernel(h->n_hel, h->tiled);
   if (!fn) return set_error(h, PWA_ERR_INVALID_ARG, "pwa_fit_fractions: n_hel out of range", cudaSuccess);
   const int R = h->n_res;
   // the per-block rows reuse the sweep's partial buffer: [2][grid][10 R + 2] doubles there, [grid][R + 1] needed here
@@ -232,7 +245,7 @@ extern "C" pwa_status pwa_fit_fractions(pwa_handle* h, const double* theta, doub
     cudaError_t ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (ce != cudaSuccess) return set_error(h, PWA_ERR_CUDA, "cudaFuncSetAttribute(k_fractions)", ce);
   }
-  fn<<<grid, FB, smem, h->stream>>>(h->smp[0], h->d_ch, theta, R, h->d_partial);
+  fn<<<grid, FB, smem, h->stream>>>(h->smp[0], h->tstore[0], h->d_ch, theta, R, h->d_partial);
   h->launches++;
   if (cudaError_t ce = cudaGetLastError()) return set_error(h, PWA_ERR_CUDA, "launch k_fractions", ce);
   k_fractions_final<<<1, FB, 0, h->stream>>>(h->d_partial, grid, R, frac);

@@ -20,6 +20,11 @@ struct pwa_handle {
   pwa::SampleDev smp[2];  // 0 = MC, 1 = data
   void* owned[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
   int* d_ch = nullptr;
+  // copy-mode handles whose shape needs 8-event tiles keep the events TILED (TiledDev, pwa_common.cuh) instead of as
+  // planes: smp[].amp / mass / weight are then null and only the tiled-aware kernels (lanes sweep PROD 4, fit fractions)
+  // may run; decided before the store is built (lanes_wants_tiled)
+  bool tiled = false;
+  pwa::TiledDev tstore[2];  // 0 = MC, 1 = data; base is owned
 
   // richer model (readings S21, S22; pwa_create_rich): the kernels work in the EXPANDED parameter space [n_res][4]
   // (every wave with its own a, phi, M, Gamma); user vectors are expanded before and contracted after a sweep
@@ -86,7 +91,7 @@ bool encode_2d(CUtensorMap* m, const void* base, unsigned long long cols, unsign
 typedef void (*lanes_fn)(const LaneArgs);
 struct LanesCombo {
   int rho, log_sw, nw, prod, tile, alt;  // resonances per lane, log2(slices per warp), compute warps per block, producer kind
-                                    // (0 warp, 2 warpgroup), events per tile (32, or 8 with the swizzled layout), and the
+                                    // (0 warp, 2 warpgroup, 4 warpgroup + tiled store), events per tile (32, or 8 with the swizzled layout), and the
                                     // entry (same rho, slices, tile) used for the modes with fewer accumulators, whose registers allow a
                                     // third compute warp per scheduler (-1: none; no entry uses one since warps keep their columns:
                                     // the 8-warp warpgroup shape then measured faster in every mode)
@@ -96,7 +101,7 @@ struct LanesCombo {
 constexpr LanesCombo kLanesCombos[] = {
     {1, 2, 15, 0, 32, -1}, {2, 3, 15, 0, 32, -1}, {3, 2, 11, 0, 32, -1}, {3, 2, 8, 2, 32, -1}, {4, 3, 8, 2, 32, -1}, {4, 3, 7, 0, 32, -1},
     {4, 4, 8, 2, 32, -1},  {4, 4, 7, 0, 32, -1},  {4, 5, 8, 2, 32, -1},  {4, 5, 7, 0, 32, -1}, {4, 4, 8, 2, 8, -1},  {4, 5, 8, 2, 8, -1},
-    {4, 3, 11, 3, 32, -1}, {5, 1, 8, 2, 32, -1}};
+    {4, 3, 11, 3, 32, -1}, {5, 1, 8, 2, 32, -1}, {4, 4, 8, 4, 8, -1},  {4, 5, 8, 4, 8, -1}};
 constexpr int kNumLanesCombos = sizeof(kLanesCombos) / sizeof(kLanesCombos[0]);
 lanes_fn lanes_kernel_h1(int combo, int mode);
 lanes_fn lanes_kernel_h2(int combo, int mode);
@@ -124,6 +129,9 @@ batch_fn batch_kernel_h4(int rho, int log_sw, int kind, int kb);
 bool batch_supported(const pwa_handle* h, int kind, int kb);
 pwa_status batch_launch(pwa_handle* h, int kind, int kb, const double* theta, const double* v, double* out);
 pwa_status lanes_configure(pwa_handle* h, std::string& why);  // sets variant = 2 on success; PWA_OK + why if unsuitable
+// Would a copy-mode handle of this shape run on 8-event tiles?  Then its store is built tiled (PROD 4 entries) and
+// *phase_mul / *tile_bytes / *off_mass / *off_wgt describe the layout (TiledDev).  PWA_TILED=0 switches it off.
+bool lanes_wants_tiled(int device, int R, int H, int C, int* phase_mul, unsigned* tile_bytes, unsigned* off_mass, unsigned* off_wgt);
 pwa_status lanes_launch(pwa_handle* h, int mode, const double* theta, const double* v, const double* skip = nullptr);
 // internal entry points used by the fit driver (enqueue only)
 pwa_status eval(pwa_handle* h, int mode, const double* theta, const double* v, double* nll, double* grad,

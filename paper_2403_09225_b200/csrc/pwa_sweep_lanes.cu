@@ -68,24 +68,19 @@ lanes_fn lanes_kernel(int H, int combo, int mode) {
   return nullptr;
 }
 
-pwa_status lanes_configure(pwa_handle* h, std::string& why) {
-  const int R = h->n_res, H = h->n_hel, C = h->n_chan;
-  for (int sidx = 0; sidx < 2; ++sidx) {
-    const SampleDev& d = h->smp[sidx];
-    if (d.n >= (1LL << 30)) { why = "sample too long for 32-bit TMA coordinates"; return PWA_OK; }
-    if ((d.stride & 1) || ((uintptr_t)d.mass & 15) || ((uintptr_t)d.amp & 15) || (d.weight && ((uintptr_t)d.weight & 15))) {
-      why = "event store not 16-byte aligned per plane (odd stride or misaligned base)";
-      return PWA_OK;
-    }
-  }
-  // candidates: every instantiated shape with capacity >= R, smallest capacity first (ties: table order); the first
-  // whose stage fits in shared memory at least twice is taken.  PWA_COMBO forces one entry (A/B runs).
-  int dev_smem = 0;
-  cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device);
-  const int forced = env_int("PWA_COMBO", -1);
+namespace {
+// shared-memory plan of one entry of kLanesCombos for a model shape
+struct Plan {
   int combo = -1, stages = 0;
   int rho = 0, log_sw = 0, nw = 0, prod = 0, tile = 0, SW = 0, RP = 0, NW = 0, nthreads = 0, nbox = 0, rows_box = 0;
   unsigned amp_bytes = 0, off_mass = 0, off_wgt = 0, stage_bytes = 0, k_bytes = 0, red_bytes = 0, xch_bytes = 0, fixed = 0;
+};
+
+// candidates: every instantiated shape with capacity >= R, smallest capacity first (ties: table order); the first
+// whose stage fits in shared memory at least twice is taken.  PWA_COMBO forces one entry (A/B runs).  tiled: only the
+// entries fed from a tiled store (PROD 4) / only the others.
+bool pick_plan(int R, int H, int C, int dev_smem, bool tiled, Plan& p, std::string& why) {
+  const int forced = env_int("PWA_COMBO", -1);
   why = H > 4 ? "no lanes-kernel instance for this n_hel" : "no lanes-kernel instance for this n_res";
   std::vector<int> order;
   for (int k = 0; k < kNumLanesCombos; ++k)
@@ -93,42 +88,94 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
   std::stable_sort(order.begin(), order.end(), [](int x, int y) {
     return (kLanesCombos[x].rho << kLanesCombos[x].log_sw) < (kLanesCombos[y].rho << kLanesCombos[y].log_sw);
   });
-  {
-    for (size_t oi = 0; oi < order.size() && combo < 0 && H <= 4; ++oi) {
-      const int k = order[oi];
-      const LanesCombo& c = kLanesCombos[k];
-      const int cap = c.rho << c.log_sw;
-      if (cap < R || !lanes_kernel(H, k, MODE_FULL)) continue;
-      rho = c.rho; log_sw = c.log_sw; nw = c.nw; prod = c.prod; tile = c.tile;
-      nthreads = lanes::lanes_threads(nw, prod);
-      SW = 1 << log_sw; RP = rho * SW;
-      NW = c.alt >= 0 ? std::max(nw, kLanesCombos[c.alt].nw) : nw;  // per-warp scratch sized for the larger of the two shapes
-      if (tile == 32) {
+  for (size_t oi = 0; oi < order.size() && p.combo < 0 && H <= 4; ++oi) {
+    const int k = order[oi];
+    const LanesCombo& c = kLanesCombos[k];
+    const int cap = c.rho << c.log_sw;
+    if ((c.prod == 4) != tiled) continue;
+    if (cap < R || !lanes_kernel(H, k, MODE_FULL)) continue;
+    p.rho = c.rho; p.log_sw = c.log_sw; p.nw = c.nw; p.prod = c.prod; p.tile = c.tile;
+    p.nthreads = lanes::lanes_threads(c.nw, c.prod);
+    p.SW = 1 << c.log_sw; p.RP = c.rho * p.SW;
+    p.NW = c.alt >= 0 ? std::max(c.nw, kLanesCombos[c.alt].nw) : c.nw;  // per-warp scratch sized for the larger of the two shapes
+    if (c.prod == 4) {
+      // the stage is the tile's image in the store: R*H amplitude rows of 128 bytes (no padding rows), masses, weights
+      p.nbox = 1; p.rows_box = R * H;
+      p.amp_bytes = (unsigned)R * H * c.tile * 16;
+      p.red_bytes = up((unsigned)(R * 10 + 2) * 8, 128);
+      p.off_mass = p.amp_bytes; p.off_wgt = p.off_mass + (unsigned)C * c.tile * 8;
+      p.stage_bytes = up(p.off_wgt + c.tile * 8, 128);
+    } else {
+      if (c.tile == 32) {
         // amplitude rows incl. the zero-filled planes of padding resonances, in nbox boxes of rows_box (<= 256) rows
-        const int rows_need = RP * H;
-        nbox = (rows_need + 255) / 256; rows_box = (rows_need + nbox - 1) / nbox;
-        amp_bytes = (unsigned)nbox * rows_box * tile * 16;
-        red_bytes = up((unsigned)nw * (R * 10 + 2) * 8, 128);  // rows for the main shape's warps only
+        const int rows_need = p.RP * H;
+        p.nbox = (rows_need + 255) / 256; p.rows_box = (rows_need + p.nbox - 1) / p.nbox;
+        p.amp_bytes = (unsigned)p.nbox * p.rows_box * c.tile * 16;
+        p.red_bytes = up((unsigned)c.nw * (R * 10 + 2) * 8, 128);  // rows for the main shape's warps only
       } else {
-        if (RP > 256) continue;  // one 3-D box [H][RP][8 events]
-        nbox = 1; rows_box = RP;
-        amp_bytes = (unsigned)H * RP * tile * 16;
-        red_bytes = up((unsigned)(R * 10 + 2) * 8, 128);  // one row: the warps add into it in turn
+        if (p.RP > 256) continue;  // one 3-D box [H][RP][8 events]
+        p.nbox = 1; p.rows_box = p.RP;
+        p.amp_bytes = (unsigned)H * p.RP * c.tile * 16;
+        p.red_bytes = up((unsigned)(R * 10 + 2) * 8, 128);  // one row: the warps add into it in turn
       }
-      off_mass = amp_bytes; off_wgt = up(off_mass + (unsigned)C * tile * 8, 128);  // TMA destinations: 128-byte aligned
-      stage_bytes = up(off_wgt + tile * 8, tile == 32 ? 128 : 1024);
-      k_bytes = up((unsigned)RP * lanes::KS * 8, 128);
-      xch_bytes = up((unsigned)NW * (32 / SW) * (4 * H + 2) * 8, 128);
-      fixed = k_bytes + red_bytes + xch_bytes + 32u * 2 * 8 + 128;
-      const int fit = (int)std::min<long long>(32, ((long long)dev_smem - fixed) / stage_bytes);
-      stages = std::min(8, fit);  // deeper rings were measured no faster (the kernel is not feed-bound); PWA_STAGES overrides
-      const int st_env = env_int("PWA_STAGES", 0);
-      if (st_env >= 2 && st_env <= fit) stages = st_env;
-      if (stages < 2) { why = "tile does not fit in shared memory"; continue; }
-      combo = k;
+      p.off_mass = p.amp_bytes; p.off_wgt = up(p.off_mass + (unsigned)C * c.tile * 8, 128);  // TMA destinations: 128-byte aligned
+      p.stage_bytes = up(p.off_wgt + c.tile * 8, c.tile == 32 ? 128 : 1024);
+    }
+    p.k_bytes = up((unsigned)p.RP * lanes::KS * 8, 128);
+    p.xch_bytes = up((unsigned)p.NW * (32 / p.SW) * (4 * H + 2) * 8, 128);
+    p.fixed = p.k_bytes + p.red_bytes + p.xch_bytes + 32u * 2 * 8 + 128;
+    const int fit = (int)std::min<long long>(32, ((long long)dev_smem - p.fixed) / p.stage_bytes);
+    p.stages = std::min(8, fit);  // deeper rings were measured no faster (the kernel is not feed-bound); PWA_STAGES overrides
+    const int st_env = env_int("PWA_STAGES", 0);
+    if (st_env >= 2 && st_env <= fit) p.stages = st_env;
+    if (p.stages < 2) { why = "tile does not fit in shared memory"; continue; }
+    p.combo = k;
+  }
+  return p.combo >= 0;
+}
+}  // namespace
+
+bool lanes_wants_tiled(int device, int R, int H, int C, int* phase_mul, unsigned* tile_bytes, unsigned* off_mass, unsigned* off_wgt) {
+  const char* e = std::getenv("PWA_TILED");
+  if (e && e[0] == '0') return false;
+  int dev_smem = 0;
+  if (cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, device) != cudaSuccess) return false;
+  std::string why;
+  Plan plain, tiled;
+  if (pick_plan(R, H, C, dev_smem, false, plain, why) && plain.tile != 8) return false;  // a 32-event tile fits: planes
+  if (!pick_plan(R, H, C, dev_smem, true, tiled, why)) return false;
+  *phase_mul = 32 / tiled.SW;
+  *tile_bytes = tiled.stage_bytes;
+  *off_mass = tiled.off_mass;
+  *off_wgt = tiled.off_wgt;
+  return true;
+}
+
+pwa_status lanes_configure(pwa_handle* h, std::string& why) {
+  const int R = h->n_res, H = h->n_hel, C = h->n_chan;
+  for (int sidx = 0; sidx < 2; ++sidx) {
+    if (h->tiled) {
+      if (h->tstore[sidx].n >= (1LL << 30)) return set_error(h, PWA_ERR_INVALID_ARG, "sample too long for the tiled store's 32-bit event index", cudaSuccess);
+      continue;
+    }
+    const SampleDev& d = h->smp[sidx];
+    if (d.n >= (1LL << 30)) { why = "sample too long for 32-bit TMA coordinates"; return PWA_OK; }
+    if ((d.stride & 1) || ((uintptr_t)d.mass & 15) || ((uintptr_t)d.amp & 15) || (d.weight && ((uintptr_t)d.weight & 15))) {
+      why = "event store not 16-byte aligned per plane (odd stride or misaligned base)";
+      return PWA_OK;
     }
   }
-  if (combo < 0) return PWA_OK;
+  int dev_smem = 0;
+  cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device);
+  Plan p;
+  if (!pick_plan(R, H, C, dev_smem, h->tiled, p, why)) {
+    if (h->tiled) return set_error(h, PWA_ERR_CUDA, "no kernel for the tiled store (internal)", cudaSuccess);
+    return PWA_OK;
+  }
+  const int combo = p.combo, stages = p.stages, rho = p.rho, nw = p.nw, prod = p.prod, tile = p.tile, SW = p.SW, RP = p.RP,
+            nthreads = p.nthreads, nbox = p.nbox, rows_box = p.rows_box;
+  const unsigned amp_bytes = p.amp_bytes, off_mass = p.off_mass, off_wgt = p.off_wgt, stage_bytes = p.stage_bytes, k_bytes = p.k_bytes,
+                 red_bytes = p.red_bytes, xch_bytes = p.xch_bytes, fixed = p.fixed;
   why.clear();
   const size_t smem = (size_t)stages * stage_bytes + fixed;
 
@@ -144,14 +191,20 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
     ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, nthr, smem);
     if (ce != cudaSuccess || occ < 1) {
       cudaGetLastError();
+      if (h->tiled) return set_error(h, PWA_ERR_CUDA, "the tiled-store kernel cannot be resident (internal)", ce);
       why = "lanes kernel cannot be resident (registers / shared memory)";
       return PWA_OK;
     }
   }
   LaneArgs& a = h->largs;
   std::memset(&a, 0, sizeof(a));
-  a.weighted = h->smp[1].weight != nullptr;
+  a.weighted = h->weighted;
   for (int sidx = 0; sidx < 2; ++sidx) {
+    if (h->tiled) {  // no tensor maps: the producer copies whole tiles
+      a.n[sidx] = h->tstore[sidx].n;
+      a.tiled[sidx] = h->tstore[sidx].base;
+      continue;
+    }
     const SampleDev& d = h->smp[sidx];
     a.n[sidx] = d.n;
     bool ok;
@@ -187,7 +240,8 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
   h->variant = 2;
   h->block = nthreads;
   h->grid = h->num_sms;
-  std::snprintf(h->variant_name, sizeof(h->variant_name), "lanes(rho=%d,sw=%d,nw=%d%s,tile=%d,stages=%d)", rho, SW, nw, prod == 2 ? "g" : "", tile, stages);
+  std::snprintf(h->variant_name, sizeof(h->variant_name), "lanes(rho=%d,sw=%d,nw=%d%s,tile=%d%s,stages=%d)", rho, SW, nw, prod >= 2 && prod != 3 ? "g" : "", tile,
+                prod == 4 ? "t" : "", stages);
   return PWA_OK;
 }
 

@@ -38,6 +38,7 @@ struct alignas(64) LaneArgs {
                        // iterations of the fit driver enqueued before the previous iteration's verdict is known)
   const int* ch;
   double* partial;  // [2][gridDim.x][R*NACC + 2]
+  const unsigned char* tiled[2];  // PROD 4: the library-owned tiled stores (TiledDev, pwa_common.cuh), tile stride = stage_bytes
   int R, C, stages;
   int nbox, rows_box;                       // amplitude rows are loaded in nbox boxes of rows_box rows (<= 256)
   unsigned stage_bytes, amp_bytes, off_mass, off_wgt;  // inside a stage: amplitude planes [rows][32 events], mass, weights
@@ -114,6 +115,13 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map
       "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(dst),
       "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar)
       : "memory");
+}
+// bulk copy of `bytes` contiguous bytes global -> shared (16-byte aligned, a multiple of 16), completion counted on an
+// mbarrier (SASS: UBLKCP)
+__device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
+               "r"(bytes), "r"(bar)
+               : "memory");
 }
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
   asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
@@ -240,7 +248,9 @@ __host__ __device__ constexpr int nacc_of() {
 //      turn): the shape a handle uses for its gradient modes beside its main shape, whose scratch it shares;
 //   2  producer warpgroup: warps 0..3 shrink to 24 registers (setmaxnreg.dec), warp 0 produces; the NW compute warps
 //      4..NW+3 grow to 240 registers (setmaxnreg.inc), so every sub-partition carries NW / 4 compute warps.
-constexpr int lanes_threads(int nw, int prod) { return (nw + (prod == 2 ? 4 : 1)) * 32; }
+//   4  as 2, fed from the library-owned TILED store (TiledDev, pwa_common.cuh) with ONE bulk copy of contiguous HBM per
+//      stage instead of tensor copies of 128-byte rows (TILE = 8 only; copy-mode handles).
+constexpr int lanes_threads(int nw, int prod) { return (nw + ((prod == 2 || prod == 4) ? 4 : 1)) * 32; }
 //
 // TILE = 32 (default): amplitude stage = [plane r*H + h][32 events], 512-byte rows, one or two 2-D boxes.
 // TILE = 8 (shapes whose 32-event tile does not fit twice in shared memory, e.g. R = 100, H = 4: 6.4 KB per event):
@@ -248,13 +258,20 @@ constexpr int lanes_threads(int nw, int prod) { return (nw + (prod == 2 ? 4 : 1)
 //   index XOR (row & 7)); the 8 lanes of a quarter-warp own consecutive resonance slots, so their 128-bit reads hit
 //   eight different chunks (conflict-free).  128-byte rows cap the TMA feed near 4.1 TB/s whatever the ring depth
 //   (measured with this layout on config 3 in NLL mode: 0.62 of the HBM peak against 1.05 for 512-byte rows), so
-//   this variant is only chosen when the 32-event tile does not fit; config 4 runs at that cap.
+//   this variant is only chosen when the 32-event tile does not fit; config 4 on a BORROWED store runs at that cap.
+// TILE = 8, PROD = 4 (the same shapes on a library-owned copy of the events): the store itself is kept as 8-event tiles
+//   in the layout of a stage (TiledDev: [resonance][h][8 events], chunk e ^ phase(r), then masses and weights), so one
+//   bulk copy of ~50 contiguous KB fills a stage: no 128-byte-row cap, no padding rows in shared memory (the lanes of
+//   padding resonances re-read the last real row and multiply it by zero constants), one stage more in the ring.
 template <int H, int RHO, int LOG_SW, int NW, int MODE, int PROD, int TILE>
 __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(const __grid_constant__ LaneArgs a) {
   constexpr int SW = 1 << LOG_SW;          // slices per warp
   constexpr int EW = 32 / SW;              // events per pass
   constexpr int NP = TILE / EW;            // passes per tile
   static_assert(TILE == 32 || (TILE == 8 && SW >= 8), "8-event tiles need at least 8 slices (swizzle phase = slice & 7)");
+  constexpr bool WG = PROD == 2 || PROD == 4;  // producer warpgroup
+  constexpr bool BULK = PROD == 4;             // stages filled by one bulk copy from the tiled store
+  static_assert(!BULK || TILE == 8, "the tiled store holds 8-event tiles");
   constexpr bool WP = mode_p(MODE), WP3 = mode_p3(MODE), WQ = mode_q(MODE);
   constexpr int QO = MODE == MODE_FULL ? 6 : 0;  // first accumulator of Q1 (FULL: after P1..P3; HVPQ: the only ones)
   constexpr int NV = (WQ ? 4 : 2) * H;  // reals exchanged per event and slice
@@ -263,7 +280,7 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
   constexpr int RP = RHO * SW;             // resonances incl. padding
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   if (a.skip != nullptr && *a.skip != 0.0) return;  // uniform over the grid
-  const int lane = threadIdx.x & 31, w = (int)(threadIdx.x >> 5) - (PROD == 2 ? 4 : 0);  // w: compute-warp index
+  const int lane = threadIdx.x & 31, w = (int)(threadIdx.x >> 5) - (WG ? 4 : 0);  // w: compute-warp index
   const int R = a.R, stages = a.stages;
   double* Ks = reinterpret_cast<double*>(smem_raw + a.off_K);    // [RP][KS]
   double* red = reinterpret_cast<double*>(smem_raw + a.off_red);  // [NW][R*NACC + 2]
@@ -304,6 +321,11 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
     const bool wg = smp == 1 && a.weighted;
     const int st = k % stages;
     const uint32_t bar = full0 + 8 * st, dst = smem_u32(smem_raw) + st * a.stage_bytes;
+    if (BULK) {  // the tile's image in the store is the stage's image
+      mbar_expect_tx(bar, a.stage_bytes);
+      bulk_load(dst, a.tiled[smp] + (size_t)(i0 / TILE) * a.stage_bytes, a.stage_bytes, bar);
+      return;
+    }
     mbar_expect_tx(bar, a.amp_bytes + (unsigned)a.C * (TILE * 8) + (wg ? TILE * 8u : 0u));
     if (TILE == 32) {
       for (int x = 0; x < a.nbox; ++x)
@@ -314,13 +336,15 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
     tma_load_2d(dst + a.off_mass, &a.tm_mass[smp], i0, 0, bar);
     if (wg) tma_load_2d(dst + a.off_wgt, &a.tm_wgt[smp], i0, 0, bar);
   };
-  if ((PROD != 2 && w == NW) || (PROD == 2 && w < 0)) {
-    if (PROD == 2) asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
-    if (lane == 0 && (PROD != 2 || w == -4) && !kNoLoad) {
-      tma_prefetch_desc(&a.tm_amp[0]);
-      tma_prefetch_desc(&a.tm_mass[0]);
-      tma_prefetch_desc(&a.tm_amp[1]);
-      tma_prefetch_desc(&a.tm_mass[1]);
+  if ((!WG && w == NW) || (WG && w < 0)) {
+    if (WG) asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
+    if (lane == 0 && (!WG || w == -4) && !kNoLoad) {
+      if (!BULK) {
+        tma_prefetch_desc(&a.tm_amp[0]);
+        tma_prefetch_desc(&a.tm_mass[0]);
+        tma_prefetch_desc(&a.tm_amp[1]);
+        tma_prefetch_desc(&a.tm_mass[1]);
+      }
       for (int k = 0; k < T; ++k) {
         if (k >= stages) mbar_wait(empty0 + 8 * (k % stages), (uint32_t)((k / stages - 1) & 1));
         issue_tile(k);
@@ -330,7 +354,7 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
   }
 
   // ======================================= compute warps ===================================================
-  if (PROD == 2) asm volatile("setmaxnreg.inc.sync.aligned.u32 240;");
+  if (WG) asm volatile("setmaxnreg.inc.sync.aligned.u32 240;");
   const int s = lane >> (5 - LOG_SW), e = lane & (EW - 1);
   double acc[RHO][NA];
   double s0 = 0.0, s1 = 0.0;
@@ -340,14 +364,21 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
     for (int q = 0; q < NA; ++q) acc[j][q] = 0.0;
   // byte offset of (resonance 0 of this slice, helicity 0, this lane's event in column 0) inside a stage; resonance j,
   // helicity h and the column add compile-time / warp-uniform constants
-  const unsigned lane_f = TILE == 32 ? (unsigned)s * (H * TILE * 16) + (unsigned)e * 16u : (unsigned)s * 128u;
+  const unsigned lane_f = TILE == 32 ? (unsigned)s * (H * TILE * 16) + (unsigned)e * 16u : BULK ? 0u : (unsigned)s * 128u;
+  // tiled store: byte offset of each own resonance's first row inside a stage; the lanes of padding resonances (slot >=
+  // R: zero constants) read the last real row instead of rows the stage does not have
+  unsigned rowoff[BULK ? RHO : 1];
+  if (BULK) {
+#pragma unroll
+    for (int j = 0; j < RHO; ++j) rowoff[j] = (unsigned)min(j * SW + s, a.R - 1) * (H * 128u);
+  }
   const double* lane_k = Ks + s * KS;
   unsigned moff[RHO];  // byte offset of each own resonance's mass row inside a stage (kept in registers: no dependent load)
 #pragma unroll
   for (int j = 0; j < RHO; ++j) moff[j] = (unsigned)__double_as_longlong(lane_k[j * (SW * KS) + 3]);
   // with the producer warpgroup the compute warps own 240 registers: keep the constants every pass needs in
   // registers instead of re-reading them from shared memory (one wavefront per 4 bytes per lane, broadcast or not)
-  constexpr bool KREG = PROD == 2 && RHO * H <= 9;  // beyond that the amplitudes G_rh themselves fill the file
+  constexpr bool KREG = WG && RHO * H <= 9;  // beyond that the amplitudes G_rh themselves fill the file
   // MODE_HVPQ holds 24 fewer accumulators per lane than the fused mode: alpha, beta live in registers there too
   // (in the fused mode the same change measured 4 % slower: no room)
   constexpr int KAB = (KREG && MODE == MODE_HVPQ) ? RHO : 0;
@@ -407,9 +438,11 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
       const bool valid = i0 + ev < n;
       if (!kNoLoad) mbar_wait(full0 + 8 * st, (uint32_t)ph);
       const unsigned char* sp = smem_raw + (size_t)st * a.stage_bytes;
-      // TILE 32: row (j SW + s) H + h, column chunk col EW + e;  TILE 8: row h RP + j SW + s, chunk (col EW + e) ^ (s & 7)
-      const unsigned char* fp = sp + lane_f + (TILE == 32 ? (col * EW) * 16 : (((col * EW + e) ^ (s & 7)) * 16));
+      // TILE 32: row (j SW + s) H + h, column chunk col EW + e;  TILE 8: row h RP + j SW + s, chunk (col EW + e) ^ (s & 7);
+      // tiled store: row (j SW + s) H + h, chunk (col EW + e) ^ ((s EW) & 7)
+      const unsigned char* fp = sp + lane_f + (TILE == 32 ? (col * EW) * 16 : (((col * EW + e) ^ ((BULK ? s * EW : s) & 7)) * 16));
       auto f_at = [&](int j, int h) {
+        if (BULK) return *reinterpret_cast<const double2*>(fp + rowoff[j] + h * 128);
         return *reinterpret_cast<const double2*>(fp + (TILE == 32 ? (j * SW * H + h) * (TILE * 16) : (h * RP + j * SW) * 128));
       };
       double wt = 1.0;

@@ -40,6 +40,8 @@ lanes_fn PWA_CAT(lanes_kernel_h, PWA_LANES_H)(int combo, int mode) {
     case 11: return for_mode<4, 5, 8, 2, 8>(mode);
     case 12: return for_mode<4, 3, 11, 3>(mode);
     case 13: return for_mode<5, 1, 8, 2>(mode);
+    case 14: return for_mode<4, 4, 8, 4, 8>(mode);
+    case 15: return for_mode<4, 5, 8, 4, 8>(mode);
   }
   return nullptr;
 }
