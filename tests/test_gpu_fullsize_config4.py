@@ -1,6 +1,7 @@
 """GPU parity at BASELINE.json's FULL config-4 size ("Big": R = 100, H = 4, 10 M MC + 1 M data events, 70.7 GB of event
-store adopted zero-copy), in the launch configuration `bench.py --config 4` times, through the C ABI (SURVEY 8(d):
-"config 4 on chunks copied back from the device"; hard part 7).
+store), through the C ABI ("config 4 on chunks copied back from the device"; hard part 7), in both launch
+configurations `bench.py --config 4` can time: the planes adopted zero-copy (`--store borrow`, tensor copies) and the
+library-owned tiled copy (`--store copy`, the default: one bulk copy per stage), which must give the same bits.
 
   * the WHOLE workload: the oracle's double build evaluates it chunk by chunk on host copies of <= 2 GB
     (oracle.raw_sums per chunk; shard additivity of the raw sums is pin P6), the chunk sums are added in 80-bit and
@@ -93,6 +94,18 @@ def test_whole_config4_against_the_oracle_chunk_by_chunk(oracle_mod, big, capsys
     assert abs(f1 - float(f0)) / max(abs(float(f0)), 1.0) < NLL_TOL and rel_l2(g1, g0) < VEC_TOL
     f2, g2, hv2 = gm.nll_grad_hvp(th, v)
     assert f2 == f and g2.tobytes() == g.tobytes() and hv2.tobytes() == hv.tobytes()  # repeat runs: same bits
+    # the library-owned tiled copy of the same 70.7 GB (what bench.py --config 4 times by default): same bits
+    torch.cuda.empty_cache()
+    tm = pwa.Model(w, device=0, borrow=False)
+    try:
+        assert "tile=8t," in pwa.pwa_kernel_variant(tm.h), pwa.pwa_kernel_variant(tm.h)
+        f3, g3, hv3 = tm.nll_grad_hvp(th, v)
+        assert f3 == f and g3.tobytes() == g.tobytes() and hv3.tobytes() == hv.tobytes()
+        f4, g4 = tm.nll_grad(th)
+        assert f4 == f1 and g4.tobytes() == g1.tobytes()
+        assert pwa.pwa_status_flags(tm.h) == 0
+    finally:
+        tm.close()
 
 
 WINDOWS = [(0, 1_031, 0, 517), (4_999_990, 2_051, 499_994, 1_027), (9_998_976, 1_024, 999_744, 256)]
@@ -108,17 +121,22 @@ def test_config4_windows_against_the_80bit_oracle(oracle_mod, big, m0, nm, d0, n
                           oracle_mod.Sample(to_np(w.data_mass[:, d0:d0 + nd].contiguous()), to_np(w.data_amp[:, :, d0:d0 + nd].contiguous()), None),
                           oracle_mod.Sample(to_np(w.mc_mass[:, m0:m0 + nm].contiguous()), to_np(w.mc_amp[:, :, m0:m0 + nm].contiguous()), None))
     f0, g0, h0 = oracle_mod.nll_grad_hvp(wm, th, v, "ld", threads=oracle_mod.max_threads())
-    h = pwa.pwa_create(w.res_chan, w.data_mass, w.data_amp, w.data_weight, w.mc_mass, w.mc_amp, borrow=True,
-                       data_first=d0, n_data=nd, mc_first=m0, n_mc=nm)
-    try:
-        dev = torch.device("cuda", 0)
-        nll = torch.zeros(1, dtype=torch.float64, device=dev)
-        g = torch.zeros(cfg.n_par, dtype=torch.float64, device=dev)
-        hv = torch.zeros(cfg.n_par, dtype=torch.float64, device=dev)
-        pwa.pwa_nll_grad_hvp(h, torch.tensor(th, device=dev), torch.tensor(v, device=dev), nll, g, hv)
-        torch.cuda.synchronize()
-        assert pwa.pwa_kernel_variant(h) == pwa.pwa_kernel_variant(gm.h)  # the variant bench.py --config 4 runs
-        assert abs(nll.item() - float(f0)) / max(abs(float(f0)), 1.0) < NLL_TOL
-        assert rel_l2(g.cpu().numpy(), g0) < VEC_TOL and rel_l2(hv.cpu().numpy(), h0) < VEC_TOL
-    finally:
-        pwa.pwa_destroy(h)
+    for borrow in (True, False):  # zero-copy window of the planes; the library's tiled copy of the window
+        h = pwa.pwa_create(w.res_chan, w.data_mass, w.data_amp, w.data_weight, w.mc_mass, w.mc_amp, borrow=borrow,
+                           data_first=d0, n_data=nd, mc_first=m0, n_mc=nm)
+        try:
+            dev = torch.device("cuda", 0)
+            nll = torch.zeros(1, dtype=torch.float64, device=dev)
+            g = torch.zeros(cfg.n_par, dtype=torch.float64, device=dev)
+            hv = torch.zeros(cfg.n_par, dtype=torch.float64, device=dev)
+            pwa.pwa_nll_grad_hvp(h, torch.tensor(th, device=dev), torch.tensor(v, device=dev), nll, g, hv)
+            torch.cuda.synchronize()
+            # the variants bench.py --config 4 runs (--store borrow / the default --store copy)
+            if borrow:
+                assert pwa.pwa_kernel_variant(h) == pwa.pwa_kernel_variant(gm.h)
+            else:
+                assert "tile=8t," in pwa.pwa_kernel_variant(h)
+            assert abs(nll.item() - float(f0)) / max(abs(float(f0)), 1.0) < NLL_TOL
+            assert rel_l2(g.cpu().numpy(), g0) < VEC_TOL and rel_l2(hv.cpu().numpy(), h0) < VEC_TOL
+        finally:
+            pwa.pwa_destroy(h)
