@@ -62,7 +62,7 @@ static sweep_fn generic_fn(int H, int mode) {
 }
 
 // blocks of the second reduction stage (phase 1 is spread over them, the last one to finish does the rest)
-static constexpr int kReduceBlocks = 8;
+static constexpr int kReduceBlocks = 16;
 
 static inline int nb_of(int R, int mode) {
   if (mode == MODE_NLL) return 0;

@@ -480,11 +480,14 @@ __global__ void __launch_bounds__(1024) k_reduce_unpack(const double* __restrict
   if (MODE == MODE_NLL) {
     for (int k = threadIdx.x; k < 4 * P; k += blockDim.x) raw[4 + k] = 0.0;
   } else {
-    for (int r = threadIdx.x; r < R; r += blockDim.x) {
+    // one thread per (resonance, sample): the two samples' unpacking (a sincos and ~150 dependent FP64 instructions each)
+    // run side by side instead of one after the other
+    for (int rs = threadIdx.x; rs < 2 * R; rs += blockDim.x) {
+      const int r = rs >> 1, sample = rs & 1;
       const int b = r / RPB, j = r - b * RPB;
       const int qoff = packed ? r * VPR : b * 32 + j * VPR;
       const double a = theta[4 * r], phi = theta[4 * r + 1], M = theta[4 * r + 2], G = theta[4 * r + 3];
-      for (int sample = 0; sample < 2; ++sample) {
+      {
         const double* q = sums + (size_t)sample * stride + qoff;
         Sums5 s;
         s.P3 = s.Q1 = s.Q2 = {0.0, 0.0};

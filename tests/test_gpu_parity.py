@@ -189,11 +189,13 @@ def test_zero_mass_resonance_on_a_ragged_tail(pwa, oracle_mod):
 
 @pytest.mark.parametrize("case,combo", [(CASES[2], 10), (CASES[2], 11), (CASES[1], 10), (CASES[0], 11), (CASES[4], 10),
                                         (CASES[2], 5), (CASES[2], 6), (CASES[2], 12), (CASES[1], 3), (CASES[1], 1), (CASES[0], 0),
-                                        (CASES[1], 2), (CASES[1], 13), (CASES[4], 13)])
+                                        (CASES[1], 2), (CASES[1], 13), (CASES[4], 13),
+                                        (CASES[2], 14), (CASES[2], 15), (CASES[1], 14), (CASES[0], 15), (CASES[3], 15)])
 def test_every_kernel_shape_matches_oracle(pwa, oracle_mod, case, combo, monkeypatch):
     """The handle normally picks one shape per (n_res, n_hel); PWA_COMBO forces another entry of kLanesCombos
-    (csrc/pwa_internal.h) so that every instantiated shape - 8-event swizzled tiles, both producer kinds, every slice
-    count - is compared with the oracle on ragged inputs, not only the ones the default choice reaches."""
+    (csrc/pwa_internal.h) so that every instantiated shape - 8-event swizzled tiles over planes and over the tiled store,
+    both producer kinds, every slice count - is compared with the oracle on ragged inputs, not only the ones the default
+    choice reaches."""
     import workloads
     cfg, w, om, _ = _case(pwa, oracle_mod, *case)
     monkeypatch.setenv("PWA_COMBO", str(combo))
@@ -203,7 +205,9 @@ def test_every_kernel_shape_matches_oracle(pwa, oracle_mod, case, combo, monkeyp
         name = pwa.pwa_kernel_variant(gm.h)
         assert name.startswith("lanes"), name
         if combo in (10, 11):
-            assert "tile=8" in name, name
+            assert "tile=8," in name, name
+        if combo in (14, 15):  # the library-owned tiled store (this handle owns a copy of the events)
+            assert "tile=8t," in name, name
         th = _thetas(cfg)[2]
         v = workloads.direction(cfg, 9).numpy()
         f0, g0, h0 = oracle_mod.nll_grad_hvp(om, th, v, "ld")
