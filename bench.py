@@ -347,6 +347,8 @@ def main():
     ap.add_argument("--batch", type=int, default=4, help="--mode nll_batch / hvp_cached_batch: evaluations per call (K)")
     ap.add_argument("--sustained-seconds", type=float, default=1.2,
                     help="length of the back-to-back run behind roofline_sustained (0 = skip)")
+    ap.add_argument("--shape", default="", help="R,H,C: another model shape on --config's recipe (kernel-shape measurements, "
+                    "profiles/r02_shapes.md; with --mc / --data); not a BASELINE.json configuration")
     ap.add_argument("--store", default="auto", choices=["auto", "borrow", "copy"],
                     help="event store of the handle: borrow = the workload's planes in place (zero copy); copy = a library-owned "
                          "copy, which shapes that need 8-event tiles keep TILED (one bulk copy per stage); auto = copy for config 4")
@@ -382,6 +384,10 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
 
     base = workloads.CONFIGS[args.config]
+    if args.shape:
+        from dataclasses import replace
+        R_, H_, C_ = (int(x) for x in args.shape.split(","))
+        base = replace(base, name=f"{base.name}, shape {args.shape}", n_res=R_, n_hel=H_, n_chan=C_, table1=False)
     cfg = base.scaled(args.mc or base.n_mc, args.data or base.n_data)
     if world > 1:  # every rank holds its own shard: same recipe, rank-specific seed
         from dataclasses import replace
@@ -553,7 +559,8 @@ def main():
     peak, peak_src = _peaks()
     sweep_avg_s = (sweep_ms / max(sweep_n, 1)) * 1e-3
     achieved = bytes_per_step / sweep_avg_s / 1e9 if sweep_n else None
-    traffic, traffic_src = (None, "stored figures are for the fused sweep") if args.mode != "nll_grad_hvp" else \
+    traffic, traffic_src = (None, "stored figures are for the fused sweep of the BASELINE.json configurations") \
+        if (args.mode != "nll_grad_hvp" or args.shape or args.mc or args.data) else \
         _stored_traffic(args.config, pwa.pwa_kernel_variant(m.h))
     line = {
         "metric": METRIC, "value": world * events_per_step * args.steps / (ms * 1e-3), "unit": UNIT,

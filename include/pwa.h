@@ -79,7 +79,13 @@ typedef struct {
   int32_t borrow;          /* PWA_MEM_DEVICE only. 1: adopt the device pointers (zero copy; the caller
                               keeps them alive and unchanged for the life of the handle; amp must be
                               16-byte aligned, mass/weight 8-byte aligned).  0: the library copies and
-                              the caller may free its buffers when pwa_create returns. */
+                              the caller may free its buffers when pwa_create returns.  The copy is laid out
+                              for the kernel the handle selects: planes as above, or - for shapes whose
+                              32-event tile does not fit twice in shared memory, e.g. n_res = 100, n_hel = 4 -
+                              8-event tiles that one bulk copy moves into shared memory (about 20 % faster
+                              there than the same kernel over borrowed planes; same results bit for bit;
+                              pwa_kernel_variant then says "tile=8t"; while pwa_create runs the copy exists
+                              beside the caller's buffers; PWA_TILED=0 in the environment keeps planes). */
   int32_t device;          /* CUDA device ordinal */
   void* stream;            /* cudaStream_t, or NULL for the legacy default stream */
 } pwa_model_desc;

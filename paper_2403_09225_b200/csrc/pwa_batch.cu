@@ -35,7 +35,7 @@ static bool pair_plan(const pwa_handle* h, PairArgs& p, size_t& smem) {
   const unsigned xch_bytes = up((unsigned)NW * 2 * EW * (4 * H + 2) * 8, 128);
   const unsigned fixed = k_bytes + red_bytes + xch_bytes + 32u * 2 * 8 + 128;
   const long long fit = ((long long)dev_smem - fixed) / h->largs.stage_bytes;
-  const int stages = (int)std::min<long long>(fit, h->largs.stages);
+  const int stages = ring_stages((int)std::min<long long>(fit, h->largs.stages));
   if (stages < 3) return false;
   p.stages = stages;
   p.off_K = (unsigned)stages * h->largs.stage_bytes;
@@ -72,6 +72,7 @@ pwa_status pair_launch(pwa_handle* h, int mode, const double* theta, const doubl
   a.v = v;
   a.skip = skip;
   a.partial = h->d_partial;
+  a.nprod = producers_for(p.stages);
   fn<<<h->grid, lanes::lanes_threads(8, 2), smem, h->stream>>>(a, p);
   if ((ce = cudaGetLastError()) != cudaSuccess) return set_error(h, PWA_ERR_CUDA, "launch two-event sweep kernel", ce);
   return PWA_OK;
@@ -103,7 +104,7 @@ static bool batch_plan(const pwa_handle* h, int kind, int kb, BatchArgs& b, size
   const unsigned xch_bytes = up(2u * NW * EW * (lanes::batch_nv(kind, kb, h->n_hel) + 2) * 8, 128);  // x 2: the paired value batch keeps two events per lane
   const unsigned fixed = k_bytes + red_bytes + xch_bytes + 32u * 2 * 8 + 128;
   const long long fit = ((long long)dev_smem - fixed) / h->largs.stage_bytes;
-  const int stages = (int)std::min<long long>(fit, h->largs.stages);
+  const int stages = ring_stages((int)std::min<long long>(fit, h->largs.stages));
   if (stages < 2) return false;
   b.stages = stages;
   b.off_K = (unsigned)stages * h->largs.stage_bytes;
@@ -158,7 +159,9 @@ pwa_status batch_launch(pwa_handle* h, int kind, int kb, const double* theta, co
   b.partial = h->d_batch;
   const bool prof = h->profiling && h->prof_used + 2 <= h->prof_events.size();
   if (prof) cudaEventRecord(h->prof_events[h->prof_used], h->stream);
-  fn<<<h->grid, lanes::lanes_threads(8, 2), smem, h->stream>>>(h->largs, b);
+  LaneArgs la = h->largs;
+  la.nprod = producers_for(b.stages);
+  fn<<<h->grid, lanes::lanes_threads(8, 2), smem, h->stream>>>(la, b);
   if (prof) {
     cudaEventRecord(h->prof_events[h->prof_used + 1], h->stream);
     h->prof_used += 2;

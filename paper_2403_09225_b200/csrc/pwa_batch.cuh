@@ -106,23 +106,31 @@ __global__ void __launch_bounds__(lanes_threads(NW, 2), 1) k_batch_lanes(const _
   // ======================================= producer ========================================================
   if (w < 0) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
-    if (lane == 0 && w == -4) {
+    // the warps of the producer warpgroup take the local tiles in turn (pwa_sweep_lanes.cuh: one issuing thread caps
+    // the ring near one tile per 800 cycles)
+    const int NPW = a.nprod, p0 = w + 4;
+    if (lane == 0 && p0 < NPW) {
       tma_prefetch_desc(&a.tm_amp[0]);
       tma_prefetch_desc(&a.tm_mass[0]);
       tma_prefetch_desc(&a.tm_amp[1]);
       tma_prefetch_desc(&a.tm_mass[1]);
-      for (int k = 0; k < T; ++k) {
-        if (k >= stages) mbar_wait(empty0 + 8 * (k % stages), (uint32_t)((k / stages - 1) & 1));
+      int st = p0 % stages, wrap = p0 / stages;  // stage of tile k and how often the ring has wrapped before it
+      for (int k = p0; k < T; k += NPW) {
+        if (wrap > 0) mbar_wait(empty0 + 8 * st, (uint32_t)((wrap - 1) & 1));
         const int smp = k >= TmB ? 1 : 0;
         const int i0 = (bk + (k - (smp ? TmB : 0)) * G) * TILE;
         const bool wg = smp == 1 && a.weighted;
-        const int st = k % stages;
         const uint32_t bar = full0 + 8 * st, dst = smem_u32(smem_raw) + st * a.stage_bytes;
         mbar_expect_tx(bar, a.amp_bytes + (unsigned)a.C * (TILE * 8) + (wg ? TILE * 8u : 0u));
         for (int x = 0; x < a.nbox; ++x)
           tma_load_2d(dst + x * a.rows_box * (TILE * 16), &a.tm_amp[smp], 2 * i0, x * a.rows_box, bar);
         tma_load_2d(dst + a.off_mass, &a.tm_mass[smp], i0, 0, bar);
         if (wg) tma_load_2d(dst + a.off_wgt, &a.tm_wgt[smp], i0, 0, bar);
+        st += NPW;
+        while (st >= stages) {
+          st -= stages;
+          ++wrap;
+        }
       }
     }
     return;

@@ -101,7 +101,10 @@ struct LanesCombo {
 constexpr LanesCombo kLanesCombos[] = {
     {1, 2, 15, 0, 32, -1}, {2, 3, 15, 0, 32, -1}, {3, 2, 11, 0, 32, -1}, {3, 2, 8, 2, 32, -1}, {4, 3, 8, 2, 32, -1}, {4, 3, 7, 0, 32, -1},
     {4, 4, 8, 2, 32, -1},  {4, 4, 7, 0, 32, -1},  {4, 5, 8, 2, 32, -1},  {4, 5, 7, 0, 32, -1}, {4, 4, 8, 2, 8, -1},  {4, 5, 8, 2, 8, -1},
-    {4, 3, 11, 3, 32, -1}, {5, 1, 8, 2, 32, -1}, {4, 4, 8, 4, 8, -1},  {4, 5, 8, 4, 8, -1}};
+    {4, 3, 11, 3, 32, -1}, {5, 1, 8, 2, 32, -1}, {4, 4, 8, 4, 8, -1},  {4, 5, 8, 4, 8, -1},
+    // finer capacities (6, 8, 20, 48): fewer padding slots for model sizes between the shapes above
+    {3, 1, 8, 2, 32, -1},  {4, 1, 8, 2, 32, -1},  {5, 2, 8, 2, 32, -1},  {3, 4, 8, 2, 32, -1}, {6, 0, 8, 2, 32, -1},
+    {3, 3, 8, 2, 32, -1},  {3, 4, 8, 2, 8, -1},   {3, 4, 8, 4, 8, -1},   {3, 5, 8, 2, 8, -1},  {3, 5, 8, 4, 8, -1}};
 constexpr int kNumLanesCombos = sizeof(kLanesCombos) / sizeof(kLanesCombos[0]);
 lanes_fn lanes_kernel_h1(int combo, int mode);
 lanes_fn lanes_kernel_h2(int combo, int mode);
@@ -128,6 +131,12 @@ batch_fn batch_kernel_h4(int rho, int log_sw, int kind, int kb);
 // one batch pass of kb (a supported count) sets / directions: sweep + reduction; false if this handle's shape has no batch kernel
 bool batch_supported(const pwa_handle* h, int kind, int kb);
 pwa_status batch_launch(pwa_handle* h, int kind, int kb, const double* theta, const double* v, double* out);
+// Warps of a producer warpgroup that issue copies (pwa_sweep_lanes.cuh): the largest count <= 4 (PWA_NPROD lowers the
+// cap) that DIVIDES the ring's stage count, so that a stage is always refilled by the same thread - the parity wait on a
+// stage's empty barrier can only tell neighbouring phases apart, which is safe only in one thread's program order.
+int producers_for(int stages);
+// a ring of `fit` stages at most: `fit`, or one stage less where that admits more producers (5 -> 4, 7 -> 6)
+int ring_stages(int fit);
 pwa_status lanes_configure(pwa_handle* h, std::string& why);  // sets variant = 2 on success; PWA_OK + why if unsuitable
 // Would a copy-mode handle of this shape run on 8-event tiles?  Then its store is built tiled (PROD 4 entries) and
 // *phase_mul / *tile_bytes / *off_mass / *off_wgt describe the layout (TiledDev).  PWA_TILED=0 switches it off.

@@ -32,6 +32,18 @@ int env_int(const char* name, int dflt) {
 inline unsigned up(unsigned x, unsigned m) { return (x + m - 1) / m * m; }
 }  // namespace
 
+int producers_for(int stages) {
+  const int cap = std::min(4, std::max(1, env_int("PWA_NPROD", 4)));
+  for (int d = cap; d > 1; --d)
+    if (stages % d == 0) return d;
+  return 1;
+}
+
+int ring_stages(int fit) {
+  if (fit >= 3 && producers_for(fit - 1) > producers_for(fit)) return fit - 1;
+  return fit;
+}
+
 bool encode_2d(CUtensorMap* m, const void* base, unsigned long long cols, unsigned long long rows,
                unsigned long long row_stride_bytes, unsigned box_cols, unsigned box_rows, bool swizzle128) {
   encode_fn fn = get_encode();
@@ -94,6 +106,11 @@ bool pick_plan(int R, int H, int C, int dev_smem, bool tiled, Plan& p, std::stri
     const int cap = c.rho << c.log_sw;
     if ((c.prod == 4) != tiled) continue;
     if (cap < R || !lanes_kernel(H, k, MODE_FULL)) continue;
+    if (forced < 0) {  // measured preference (profiles/r02_shapes.md); a forced entry is taken as it is
+      // beyond 32 resonances a 32-event stage fits only a few times: the 8-event tiles (8 stages, one column per warp)
+      // were faster in every shape measured (R = 33 .. 128, H = 1 .. 4), also at a larger padded capacity
+      if (R > 32 && c.tile == 32) continue;
+    }
     p.rho = c.rho; p.log_sw = c.log_sw; p.nw = c.nw; p.prod = c.prod; p.tile = c.tile;
     p.nthreads = lanes::lanes_threads(c.nw, c.prod);
     p.SW = 1 << c.log_sw; p.RP = c.rho * p.SW;
@@ -126,6 +143,7 @@ bool pick_plan(int R, int H, int C, int dev_smem, bool tiled, Plan& p, std::stri
     p.fixed = p.k_bytes + p.red_bytes + p.xch_bytes + 32u * 2 * 8 + 128;
     const int fit = (int)std::min<long long>(32, ((long long)dev_smem - p.fixed) / p.stage_bytes);
     p.stages = std::min(8, fit);  // deeper rings were measured no faster (the kernel is not feed-bound); PWA_STAGES overrides
+    if (c.prod == 2 || c.prod == 4) p.stages = ring_stages(p.stages);
     const int st_env = env_int("PWA_STAGES", 0);
     if (st_env >= 2 && st_env <= fit) p.stages = st_env;
     if (p.stages < 2) { why = "tile does not fit in shared memory"; continue; }
@@ -226,6 +244,7 @@ pwa_status lanes_configure(pwa_handle* h, std::string& why) {
   }
   a.ch = h->d_ch;
   a.R = R; a.C = C; a.stages = stages;
+  a.nprod = producers_for(stages);
   a.nbox = nbox; a.rows_box = rows_box;
   a.stage_bytes = stage_bytes; a.amp_bytes = amp_bytes; a.off_mass = off_mass; a.off_wgt = off_wgt;
   a.off_K = (unsigned)stages * stage_bytes;

@@ -40,6 +40,7 @@ struct alignas(64) LaneArgs {
   double* partial;  // [2][gridDim.x][R*NACC + 2]
   const unsigned char* tiled[2];  // PROD 4: the library-owned tiled stores (TiledDev, pwa_common.cuh), tile stride = stage_bytes
   int R, C, stages;
+  int nprod;  // warps of the producer warpgroup that issue copies (1 .. 4; PWA_NPROD)
   int nbox, rows_box;                       // amplitude rows are loaded in nbox boxes of rows_box rows (<= 256)
   unsigned stage_bytes, amp_bytes, off_mass, off_wgt;  // inside a stage: amplitude planes [rows][32 events], mass, weights
   unsigned off_K, off_red, off_bar, off_xch;  // after the stages; xch: [NW][32/SW events][4H + 2] doubles
@@ -314,12 +315,11 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
   const int T = TmB + TdB;
 
   // ======================================= producer ========================================================
-  // copies of local tile k into its stage; the caller has made sure the stage is free
-  auto issue_tile = [&](int k) {
+  // copies of local tile k into its stage st; the caller has made sure the stage is free
+  auto issue_tile = [&](int k, int st) {
     const int smp = k >= TmB ? 1 : 0;
     const int i0 = (b + (k - (smp ? TmB : 0)) * G) * TILE;
     const bool wg = smp == 1 && a.weighted;
-    const int st = k % stages;
     const uint32_t bar = full0 + 8 * st, dst = smem_u32(smem_raw) + st * a.stage_bytes;
     if (BULK) {  // the tile's image in the store is the stage's image
       mbar_expect_tx(bar, a.stage_bytes);
@@ -338,16 +338,27 @@ __global__ void __launch_bounds__(lanes_threads(NW, PROD), 1) k_sweep_lanes(cons
   };
   if ((!WG && w == NW) || (WG && w < 0)) {
     if (WG) asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
-    if (lane == 0 && (!WG || w == -4) && !kNoLoad) {
+    // The warps of a producer warpgroup take the local tiles in turn (warp p: tiles p, p + NPW, ...): one thread issuing
+    // every tile's copies caps the ring near one tile per 800 cycles, which bounds the shapes with small tiles (a few
+    // KB per 32 events) below the feed and below their arithmetic.  Tiles need no order among themselves: a stage's
+    // empty barrier alone guards its reuse.
+    const int NPW = WG ? a.nprod : 1, p0 = WG ? w + 4 : 0;
+    if (lane == 0 && p0 < NPW && !kNoLoad) {
       if (!BULK) {
         tma_prefetch_desc(&a.tm_amp[0]);
         tma_prefetch_desc(&a.tm_mass[0]);
         tma_prefetch_desc(&a.tm_amp[1]);
         tma_prefetch_desc(&a.tm_mass[1]);
       }
-      for (int k = 0; k < T; ++k) {
-        if (k >= stages) mbar_wait(empty0 + 8 * (k % stages), (uint32_t)((k / stages - 1) & 1));
-        issue_tile(k);
+      int st = p0 % stages, wrap = p0 / stages;  // stage of tile k and how often the ring has wrapped before it
+      for (int k = p0; k < T; k += NPW) {
+        if (wrap > 0) mbar_wait(empty0 + 8 * st, (uint32_t)((wrap - 1) & 1));
+        issue_tile(k, st);
+        st += NPW;
+        while (st >= stages) {
+          st -= stages;
+          ++wrap;
+        }
       }
     }
     return;

@@ -42,6 +42,16 @@ lanes_fn PWA_CAT(lanes_kernel_h, PWA_LANES_H)(int combo, int mode) {
     case 13: return for_mode<5, 1, 8, 2>(mode);
     case 14: return for_mode<4, 4, 8, 4, 8>(mode);
     case 15: return for_mode<4, 5, 8, 4, 8>(mode);
+    case 16: return for_mode<3, 1, 8, 2>(mode);
+    case 17: return for_mode<4, 1, 8, 2>(mode);
+    case 18: return for_mode<5, 2, 8, 2>(mode);
+    case 19: return for_mode<3, 4, 8, 2>(mode);
+    case 20: return for_mode<6, 0, 8, 2>(mode);
+    case 21: return for_mode<3, 3, 8, 2>(mode);
+    case 22: return for_mode<3, 4, 8, 2, 8>(mode);
+    case 23: return for_mode<3, 4, 8, 4, 8>(mode);
+    case 24: return for_mode<3, 5, 8, 2, 8>(mode);
+    case 25: return for_mode<3, 5, 8, 4, 8>(mode);
   }
   return nullptr;
 }
@@ -77,6 +87,10 @@ batch_fn batch_for(int kind, int kb) {
 }  // namespace
 batch_fn PWA_CAT(batch_kernel_h, PWA_LANES_H)(int rho, int log_sw, int kind, int kb) {
   if (rho == 5 && log_sw == 1) return batch_for<5, 1>(kind, kb);
+  if (rho == 3 && log_sw == 1) return batch_for<3, 1>(kind, kb);
+  if (rho == 4 && log_sw == 1) return batch_for<4, 1>(kind, kb);
+  if (rho == 5 && log_sw == 2) return batch_for<5, 2>(kind, kb);
+  if (rho == 3 && log_sw == 3) return batch_for<3, 3>(kind, kb);
   if (rho == 3 && log_sw == 2) return batch_for<3, 2>(kind, kb);
   if (rho == 4 && log_sw == 3) return batch_for<4, 3>(kind, kb);
   // 16 or 32 slices (R > 32) leave fewer passes per tile than warps: no fixed column; those shapes take single passes

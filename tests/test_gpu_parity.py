@@ -190,7 +190,9 @@ def test_zero_mass_resonance_on_a_ragged_tail(pwa, oracle_mod):
 @pytest.mark.parametrize("case,combo", [(CASES[2], 10), (CASES[2], 11), (CASES[1], 10), (CASES[0], 11), (CASES[4], 10),
                                         (CASES[2], 5), (CASES[2], 6), (CASES[2], 12), (CASES[1], 3), (CASES[1], 1), (CASES[0], 0),
                                         (CASES[1], 2), (CASES[1], 13), (CASES[4], 13),
-                                        (CASES[2], 14), (CASES[2], 15), (CASES[1], 14), (CASES[0], 15), (CASES[3], 15)])
+                                        (CASES[2], 14), (CASES[2], 15), (CASES[1], 14), (CASES[0], 15), (CASES[3], 15),
+                                        (CASES[4], 16), (CASES[4], 17), (CASES[4], 20), (CASES[0], 16), (CASES[1], 18), (CASES[1], 21),
+                                        (CASES[2], 19), (CASES[2], 22), (CASES[2], 23), (CASES[2], 24), (CASES[2], 25), (CASES[1], 23)])
 def test_every_kernel_shape_matches_oracle(pwa, oracle_mod, case, combo, monkeypatch):
     """The handle normally picks one shape per (n_res, n_hel); PWA_COMBO forces another entry of kLanesCombos
     (csrc/pwa_internal.h) so that every instantiated shape - 8-event swizzled tiles over planes and over the tiled store,
@@ -204,9 +206,9 @@ def test_every_kernel_shape_matches_oracle(pwa, oracle_mod, case, combo, monkeyp
     try:
         name = pwa.pwa_kernel_variant(gm.h)
         assert name.startswith("lanes"), name
-        if combo in (10, 11):
+        if combo in (10, 11, 22, 24):
             assert "tile=8," in name, name
-        if combo in (14, 15):  # the library-owned tiled store (this handle owns a copy of the events)
+        if combo in (14, 15, 23, 25):  # the library-owned tiled store (this handle owns a copy of the events)
             assert "tile=8t," in name, name
         th = _thetas(cfg)[2]
         v = workloads.direction(cfg, 9).numpy()
