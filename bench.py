@@ -67,6 +67,7 @@ class ClockSampler:
             self.source = "nvml"
             self.thread = threading.Thread(target=self._poll_nvml, daemon=True)
             self.thread.start()
+            self._wait_first_sample()
             return
         except Exception:
             self.source = None
@@ -80,6 +81,14 @@ class ClockSampler:
             return
         self.thread = threading.Thread(target=self._read_smi, daemon=True)
         self.thread.start()
+        self._wait_first_sample()
+
+    def _wait_first_sample(self, timeout_s: float = 3.0):
+        """The first NVML query of a process can take tens of milliseconds: a timed region must not start (and end)
+        before the sampler has delivered anything."""
+        t_end = time.time() + timeout_s
+        while not self.rows and time.time() < t_end:
+            time.sleep(0.001)
 
     def _poll_nvml(self):
         nv = self.nv
