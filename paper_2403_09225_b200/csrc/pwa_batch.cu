@@ -35,8 +35,8 @@ static bool pair_plan(const pwa_handle* h, PairArgs& p, size_t& smem) {
   const unsigned xch_bytes = up((unsigned)NW * 2 * EW * (4 * H + 2) * 8, 128);
   const unsigned fixed = k_bytes + red_bytes + xch_bytes + 32u * 2 * 8 + 128;
   const long long fit = ((long long)dev_smem - fixed) / h->largs.stage_bytes;
-  const int stages = ring_stages((int)std::min<long long>(fit, h->largs.stages));
-  if (stages < 3) return false;
+  const int stages = ring_stages((int)std::min<long long>(fit, h->largs.stages), 2);  // two tiles are consumed at a time
+  if (stages < 4) return false;
   p.stages = stages;
   p.off_K = (unsigned)stages * h->largs.stage_bytes;
   p.off_red = p.off_K + k_bytes;
@@ -104,7 +104,9 @@ static bool batch_plan(const pwa_handle* h, int kind, int kb, BatchArgs& b, size
   const unsigned xch_bytes = up(2u * NW * EW * (lanes::batch_nv(kind, kb, h->n_hel) + 2) * 8, 128);  // x 2: the paired value batch keeps two events per lane
   const unsigned fixed = k_bytes + red_bytes + xch_bytes + 32u * 2 * 8 + 128;
   const long long fit = ((long long)dev_smem - fixed) / h->largs.stage_bytes;
-  const int stages = ring_stages((int)std::min<long long>(fit, h->largs.stages));
+  // tiles consumed at the same time: the paired value batch of the 8-slice shape takes two, the others 8 / passes per tile
+  const int group = (kind == BK_NLL && c.log_sw == 3) ? 2 : std::max(1, NW / (32 / EW));
+  const int stages = ring_stages((int)std::min<long long>(fit, h->largs.stages), group);
   if (stages < 2) return false;
   b.stages = stages;
   b.off_K = (unsigned)stages * h->largs.stage_bytes;

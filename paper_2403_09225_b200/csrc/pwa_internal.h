@@ -135,8 +135,13 @@ pwa_status batch_launch(pwa_handle* h, int kind, int kb, const double* theta, co
 // cap) that DIVIDES the ring's stage count, so that a stage is always refilled by the same thread - the parity wait on a
 // stage's empty barrier can only tell neighbouring phases apart, which is safe only in one thread's program order.
 int producers_for(int stages);
-// a ring of `fit` stages at most: `fit`, or one stage less where that admits more producers (5 -> 4, 7 -> 6)
-int ring_stages(int fit);
+// A ring of `fit` stages at most.  `group` = tiles that DIFFERENT warps consume at the same time (shapes whose warps keep
+// their column: compute warps / passes per tile): the stage count must be a multiple of it, so that the tiles t and
+// t + stages, which share a stage, are consumed by the same warps one after the other - a consumer that starts to wait
+// for a stage's next phase before the current one has completed would be let through by the parity wait.  Among the
+// admissible counts: `fit` rounded down, or one step less where that admits more producers (5 -> 4, 7 -> 6).
+// Returns 0 if no admissible count >= 2 exists.
+int ring_stages(int fit, int group);
 pwa_status lanes_configure(pwa_handle* h, std::string& why);  // sets variant = 2 on success; PWA_OK + why if unsuitable
 // Would a copy-mode handle of this shape run on 8-event tiles?  Then its store is built tiled (PROD 4 entries) and
 // *phase_mul / *tile_bytes / *off_mass / *off_wgt describe the layout (TiledDev).  PWA_TILED=0 switches it off.

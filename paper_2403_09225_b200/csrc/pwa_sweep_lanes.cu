@@ -39,9 +39,14 @@ int producers_for(int stages) {
   return 1;
 }
 
-int ring_stages(int fit) {
-  if (fit >= 3 && producers_for(fit - 1) > producers_for(fit)) return fit - 1;
-  return fit;
+int ring_stages(int fit, int group) {
+  if (group < 1) group = 1;
+  const int lo = std::max(2, group);
+  int best = fit - fit % group;
+  if (best < lo) return 0;
+  const int less = best - group;
+  if (less >= lo && less >= 3 && producers_for(less) > producers_for(best)) best = less;
+  return best;
 }
 
 bool encode_2d(CUtensorMap* m, const void* base, unsigned long long cols, unsigned long long rows,
@@ -142,10 +147,11 @@ bool pick_plan(int R, int H, int C, int dev_smem, bool tiled, Plan& p, std::stri
     p.xch_bytes = up((unsigned)p.NW * (32 / p.SW) * (4 * H + 2) * 8, 128);
     p.fixed = p.k_bytes + p.red_bytes + p.xch_bytes + 32u * 2 * 8 + 128;
     const int fit = (int)std::min<long long>(32, ((long long)dev_smem - p.fixed) / p.stage_bytes);
-    p.stages = std::min(8, fit);  // deeper rings were measured no faster (the kernel is not feed-bound); PWA_STAGES overrides
-    if (c.prod == 2 || c.prod == 4) p.stages = ring_stages(p.stages);
+    // warps that keep their column (NW a multiple of the passes per tile) consume NW / NP tiles at the same time
+    const int NP = c.tile / (32 / p.SW), group = (c.nw % NP == 0) ? c.nw / NP : 1;
+    p.stages = ring_stages(std::min(8, fit), group);  // deeper rings were measured no faster; PWA_STAGES overrides
     const int st_env = env_int("PWA_STAGES", 0);
-    if (st_env >= 2 && st_env <= fit) p.stages = st_env;
+    if (st_env >= 2 && st_env <= fit && st_env % group == 0) p.stages = st_env;
     if (p.stages < 2) { why = "tile does not fit in shared memory"; continue; }
     p.combo = k;
   }

@@ -58,3 +58,14 @@ def test_fit_mode_line():
     if "best" in d:
         b = d["best"]
         assert abs(b["nll"] - b["oracle_nll_at_best_theta"]) <= 1e-9 * abs(b["nll"])
+
+
+def test_shape_and_store_flags():
+    """--shape (another model shape on the config's recipe) and --store copy (library-owned copy; tiled for shapes that
+    need 8-event tiles): same contract line, no stored traffic figure for a non-BASELINE shape."""
+    d = _run("--shape", "40,4,3", "--mc", "60000", "--data", "6000", "--store", "copy", "--steps", "3", "--warmup", "3",
+             "--no-cpu-baseline", "--sustained-seconds", "0")
+    assert "shape 40,4,3" in d["config"]["workload"] and "R=40 H=4 C=3" in d["config"]["workload"]
+    assert d["config"]["store"] == "library-owned copy" and "tile=8t," in d["config"]["kernel_variant"]
+    assert d["roofline"]["traffic"] is None and d["roofline"]["bytes_per_launch"] == 66000 * (16 * 40 * 4 + 8 * 3) + 6000 * 8
+    assert d["clocks"]["sm_mhz"] is not None

@@ -225,6 +225,42 @@ def test_every_kernel_shape_matches_oracle(pwa, oracle_mod, case, combo, monkeyp
         gm.close()
 
 
+@pytest.mark.parametrize("case", [CASES[1], CASES[2], CASES[3]])
+@pytest.mark.parametrize("stages,nprod", [(0, 1), (0, 2), (0, 3), (2, 4), (3, 4), (4, 4), (5, 4), (6, 4), (7, 4)])
+def test_ring_depth_and_producer_count_do_not_change_a_bit(pwa, oracle_mod, case, stages, nprod, monkeypatch):
+    """The ring of stages is filled by up to four producer threads; their count must divide the stage
+    count so that a stage is always refilled by the same thread, and the stage count must be a multiple of the tiles
+    that different warps consume at the same time.  Whatever PWA_STAGES / PWA_NPROD ask for - rings shorter than the
+    producer count, odd depths (a depth the shape cannot run with is ignored) - the results are the default
+    configuration's, bit for bit, in every mode (the arithmetic does not depend on who copied a tile)."""
+    import workloads
+    cfg, w, om, gm = _case(pwa, oracle_mod, *case)
+    th, v = _thetas(cfg)[1], workloads.direction(cfg, 2).numpy()
+    want = (gm.nll_grad_hvp(th, v), gm.nll(th), gm.nll_grad(th), gm.nll_grad_for_hvp(th), gm.hvp_cached(v))
+    if stages:
+        monkeypatch.setenv("PWA_STAGES", str(stages))
+    monkeypatch.setenv("PWA_NPROD", str(nprod))
+    other = pwa.Model(w)
+    monkeypatch.delenv("PWA_NPROD")
+    if stages:
+        monkeypatch.delenv("PWA_STAGES")
+    try:
+        name = pwa.pwa_kernel_variant(other.h)
+        assert name.startswith("lanes"), name
+        got = (other.nll_grad_hvp(th, v), other.nll(th), other.nll_grad(th), other.nll_grad_for_hvp(th), other.hvp_cached(v))
+        flat = lambda r: np.concatenate([np.atleast_1d(np.asarray(x, dtype=np.float64)).ravel() for x in (r if isinstance(r, tuple) else (r,))])
+        # a ring of fewer than four stages has no two-events-per-lane kernel (config-3 shape): the one-event kernel of the
+        # same shape sums in another order - equal to rounding there, the same bits everywhere else
+        other_kernel = case == CASES[2] and stages in (2, 3)
+        for a, b in zip(got, want):
+            if other_kernel:
+                assert rel_l2(flat(a), flat(b)) < 1e-11, name
+            else:
+                assert flat(a).tobytes() == flat(b).tobytes(), name
+    finally:
+        other.close()
+
+
 def test_one_event_fused_kernel_of_the_config3_shape(pwa, oracle_mod, monkeypatch):
     """The fused calls of the 4 x 8-slice shape run the two-events-per-lane kernel (csrc/pwa_sweep_pair.cuh); PWA_PAIR=0
     keeps the one-event kernel of the same shape reachable - both against the oracle, and against each other (the two
