@@ -1,5 +1,6 @@
 """Edge shapes through the C ABI against the oracle: the smallest and largest models each kernel family serves, event
-counts below one tile, one event, the shape-selection boundaries (capacity 4 / 12 / 16 / 32 / 64 / 128, more than 128
+counts below one tile, one event, the shape-selection boundaries (capacity 4 / 6 / 8 / 10 / 12 / 16 / 20 / 24 / 32 / 48 / 64 /
+96 / 128, more than 128
 resonances and more than 4 helicities on the generic kernel), weighted and unweighted data."""
 import numpy as np
 import pytest
@@ -16,7 +17,12 @@ SHAPES = [(1, 1, 1, 1, 1, False), (1, 1, 1, 33, 65, True), (2, 4, 1, 7, 100, Tru
           (64, 1, 3, 50, 600, False), (65, 3, 2, 40, 400, True), (128, 4, 3, 33, 300, False), (129, 2, 3, 33, 300, True),
           (6, 5, 2, 50, 500, True), (3, 8, 1, 20, 333, False),
           # the two-events-per-lane fused kernel (13 <= R <= 32, H <= 2): H = 1, one event, fewer tiles than blocks and warps
-          (20, 1, 2, 70, 900, True), (30, 2, 3, 1, 1, False), (25, 2, 1, 33, 65, True), (32, 1, 3, 31, 4777, False)]
+          (20, 1, 2, 70, 900, True), (30, 2, 3, 1, 1, False), (25, 2, 1, 33, 65, True), (32, 1, 3, 31, 4777, False),
+          # the capacity boundaries of the finer shape grid (6, 8, 20, 24 slots on 32-event tiles; 48, 96 on 8-event tiles)
+          (6, 2, 1, 100, 1001, True), (7, 3, 2, 65, 700, False), (8, 4, 2, 9, 333, True), (9, 2, 3, 40, 401, False),
+          (17, 2, 3, 100, 999, True), (20, 4, 3, 33, 515, False), (21, 3, 2, 70, 640, True), (24, 2, 3, 129, 1025, False),
+          (34, 2, 3, 50, 600, True), (48, 4, 2, 17, 300, False), (49, 1, 3, 64, 512, True), (96, 2, 3, 33, 257, False),
+          (97, 3, 2, 20, 200, True)]
 
 
 @pytest.fixture(scope="module")
