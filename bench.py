@@ -408,7 +408,13 @@ def main():
     store = args.store if args.store != "auto" else ("copy" if args.config == 4 else "borrow")
     if store == "copy":
         torch.cuda.empty_cache()  # the library's copy is allocated beside the workload (config 4: 2 x 70.7 GB of 180 GB)
-    m = pwa.Model(w, device=local, borrow=store == "borrow")
+    try:
+        m = pwa.Model(w, device=local, borrow=store == "borrow")
+    except pwa.PwaError as e:  # no room for a second copy beside the workload: time the borrowed planes instead
+        if store != "copy" or e.status != pwa.PWA_ERR_OOM:
+            raise
+        store = "borrow"
+        m = pwa.Model(w, device=local, borrow=True)
     P = m.P
     th_np = workloads.random_start(base, 0).numpy()
     v_np = workloads.direction(base, 0).numpy()
