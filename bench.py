@@ -146,15 +146,40 @@ class ClockSampler:
                 self.proc.kill()
 
 
+def _strip_comments(src: str) -> str:
+    """C / C++ source without its comments and with runs of white space collapsed (string and character literals are
+    kept as they are): what the compiler sees, so that a comment-only edit does not invalidate a stored capture."""
+    out, i, n = [], 0, len(src)
+    while i < n:
+        c = src[i]
+        if c in "\"'":  # literal: copy up to the closing quote
+            j = i + 1
+            while j < n and src[j] != c:
+                j += 2 if src[j] == "\\" else 1
+            out.append(src[i:j + 1])
+            i = j + 1
+        elif src.startswith("//", i):
+            j = src.find("\n", i)
+            i = n if j < 0 else j
+        elif src.startswith("/*", i):
+            j = src.find("*/", i + 2)
+            i = n if j < 0 else j + 2
+            out.append(" ")
+        else:
+            out.append(c)
+            i += 1
+    return " ".join("".join(out).split())
+
+
 def _csrc_digest() -> str:
-    """sha256 over the sources of the sweep kernel and its launch configuration: ties a stored ncu traffic figure to
-    the code it was captured on."""
+    """sha256 over the sources (comments and white space aside) of the sweep kernel and its launch configuration: ties a
+    stored ncu traffic figure to the code it was captured on."""
     import hashlib
     d = os.path.join(ROOT, "paper_2403_09225_b200", "csrc")
     hsh = hashlib.sha256()
     for name in ("pwa_common.cuh", "pwa_kernels.cuh", "pwa_sweep_lanes.cuh", "pwa_sweep_lanes.cu", "pwa_sweep_pair.cuh"):
-        with open(os.path.join(d, name), "rb") as f:
-            hsh.update(name.encode() + b"\0" + f.read())
+        with open(os.path.join(d, name), "r", encoding="utf-8") as f:
+            hsh.update(name.encode() + b"\0" + _strip_comments(f.read()).encode())
     return hsh.hexdigest()[:16]
 
 

@@ -1,11 +1,12 @@
 // pwa_sweep_lanes.cuh - the warp-autonomous sweep kernel of the hot path (SURVEY §8(a) rows a-1 .. a-7), sm_100a.
 //
-// Work decomposition.  A tile is 32 consecutive events.  Tiles reach shared memory through a ring of stages
-// filled by one producer thread with TMA tensor copies (cp.async.bulk.tensor.2d): one box of 32 events x all R*H
-// amplitude planes (512 contiguous bytes per plane; narrower boxes were measured to cap the feed near 4.1 TB/s), one
-// box for the mass planes, one for the weights; full[stage] / empty[stage] mbarriers track the ring; events beyond
-// the ragged end and the planes of padding resonances are zero-filled by the TMA unit.  Every F element is read
-// from HBM exactly once and is consumed by exactly one thread.
+// Work decomposition.  A tile is 32 consecutive events (8 for the large shapes, see k_sweep_lanes).  Tiles reach shared
+// memory through a ring of stages filled by up to four producer threads (one per warp of the producer warpgroup, taking
+// the tiles in turn) with TMA tensor copies (cp.async.bulk.tensor.2d): one box of 32 events x all R*H amplitude planes
+// (512 contiguous bytes per plane; narrower boxes were measured to cap the feed near 4.1 TB/s), one box for the mass
+// planes, one for the weights - or, from a library-owned tiled store, with ONE bulk copy per stage; full[stage] /
+// empty[stage] mbarriers track the ring; events beyond the ragged end and the planes of padding resonances are
+// zero-filled by the TMA unit.  Every F element is read from HBM exactly once and is consumed by exactly one thread.
 //
 // A compute warp works on one "pass" at a time: EW = 32 / SW consecutive events of a tile, the R resonances dealt
 // over SW "slices" of RHO resonances each.  lane = s * EW + e (slice s, event e); lane (s, e) owns the resonances

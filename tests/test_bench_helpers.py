@@ -51,3 +51,11 @@ def test_clock_sampler_window_picks_the_samples_of_the_region():
     assert w["samples"] == 2 and "note" in w
     s.source = None
     assert s.window(t0, t0 + 1)["sm_mhz"] is None
+
+
+def test_digest_ignores_comments_and_white_space_but_not_code():
+    import bench
+    a = 'int a = 1; // c1\n/* c2\n   c3 */ const char* s = "x // kept /* kept */"; char q = \'"\';  asm("mov // x;");\n\tint   b;'
+    assert bench._strip_comments(a) == 'int a = 1; const char* s = "x // kept /* kept */"; char q = \'"\'; asm("mov // x;"); int b;'
+    assert bench._strip_comments("x = 1; // one\n") == bench._strip_comments("x  =  1;   /* two */")
+    assert bench._strip_comments("x = 1;") != bench._strip_comments("x = 2;")
